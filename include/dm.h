@@ -1,0 +1,149 @@
+/*
+ * dm.h -- C ABI of the B200-native multi-mode difference-map (DM) iteration.
+ *
+ * What it computes: Section II of arXiv:1808.10375, eqs. (1)-(7):
+ * for every view j and mode pair (k,l) the exit wave psi_jkl = P_k * O_l|window (eq. 2,
+ * PAPER.md:43) is updated by eq. (3) with the constrained Fourier
+ * transform of eq. (4), then the object is updated by eq. (6)
+ * (PAPER.md:60), the probe by eq. (5), and one row of convergence errors
+ * (eq. (7)) is appended.  Readings of everything the paper leaves open
+ * (order of the updates, beta, regularisers, FFT convention, error definitions) are the
+ * table "Readings" in DESIGN.md; this header only states argument meaning.
+ *
+ * Conventions
+ *   - every pointer says HOST or DEV.  DEV = device memory of the current CUDA device,
+ *     owned by the caller (PyTorch in this repo); the library never frees or reallocates
+ *     caller memory and allocates no device memory itself: all state lives in the
+ *     workspace the caller lends with dm_plan_set_workspace.
+ *   - complex arrays are interleaved float pairs (re,im) = complex64, row-major.
+ *       probe   c64 [K][N][N]          object  c64 [L][obj_h][obj_w]
+ *       psi     c64 [n_views][K][L][N][N]
+ *       intensities f32 [n_views][N][N], zero frequency (DC) at index [0][0], never fftshifted
+ *   - positions int32 [n_views][2] = (y0,x0): top-left corner of view j's N x N object
+ *     window; probe pixel (ry,rx) meets object pixel (y0+ry, x0+rx).  Integer pixels only.
+ *   - `stream` is a cudaStream_t passed as void* (NULL = default stream).  Work is enqueued
+ *     asynchronously unless the function says "syncs".
+ *   - no exception, abort or exit crosses this boundary: every call returns a dm_status.
+ *     dm_last_error(plan) gives a text for the last non-OK status of that plan.
+ *     Asynchronous device faults surface as DM_ERR_CUDA at the next syncing call.
+ *   - thread safety: one plan may be used from one host thread at a time.
+ */
+#ifndef DM_B200_H
+#define DM_B200_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct dm_plan dm_plan; /* opaque, owned by the library */
+
+typedef enum {
+    DM_OK = 0,
+    DM_ERR_INVALID_ARG = 1,   /* null pointer, non-positive size, value out of range        */
+    DM_ERR_OUT_OF_BOUNDS = 2, /* a view window is not inside [0,obj_h) x [0,obj_w)          */
+    DM_ERR_UNSUPPORTED = 3,   /* N not in {64,128,256,512}, K*L > 8, odd obj_w              */
+    DM_ERR_NO_DATA = 4,       /* dm_iterate / getters before dm_set_data                    */
+    DM_ERR_WORKSPACE = 5,     /* workspace missing, too small, misaligned, error table full */
+    DM_ERR_CUDA = 6           /* a CUDA runtime call failed; text in dm_last_error          */
+} dm_status;
+
+typedef enum {
+    DM_PARAM_BETA = 0,        /* beta of eq. (3), in [0,1]; default 1.0                      */
+    DM_PARAM_ALPHA_OBJ = 1,   /* relative inertial factor a_O >= 0 of eq. (6); default 1e-3  */
+    DM_PARAM_ALPHA_PROBE = 2, /* relative inertial factor a_P >= 0 of eq. (5); default 1e-3  */
+    DM_PARAM_EPS_F = 3,       /* zero guard in eq. (4): scale = amp/sqrt(S+eps); default 1e-30 */
+    DM_PARAM_PATH = 4         /* 0 = auto (default), 1 = force the staged (L2-scratch) path,
+                                 2 = force the fused per-frame path (DM_ERR_UNSUPPORTED at
+                                 dm_set_data if N > 128)                                     */
+} dm_param;
+
+/* Build the plan (HOST only, no CUDA call): validates, copies `positions` (HOST,
+ * int32 [n_views][2]), builds the scan-window table and the per-object-tile coverage
+ * lists (step S0 of DESIGN.md; r_j of eq. (2)).
+ * Errors: INVALID_ARG (null, sizes <= 0), UNSUPPORTED (N, K*L, odd obj_w),
+ * OUT_OF_BOUNDS (first offending view is named in dm_last_error of a NULL plan).    */
+dm_status dm_plan_create(dm_plan **out, int N, int n_views, int K, int L, int obj_h, int obj_w,
+                         const int32_t *positions);
+
+/* Set a parameter.  Must precede dm_set_data (INVALID_ARG afterwards or out of range). */
+dm_status dm_plan_set_param(dm_plan *plan, dm_param which, double value);
+
+/* Bytes of device workspace the plan needs (psi, sqrt(I), P/O double buffers, tables,
+ * partial sums, error table, L2 scratch of the staged path).                          */
+dm_status dm_plan_workspace_bytes(const dm_plan *plan, size_t *bytes);
+
+/* Lend the workspace: DEV pointer, 256-byte aligned, >= dm_plan_workspace_bytes.  Borrowed
+ * until dm_plan_destroy; contents are the library's.                                   */
+dm_status dm_plan_set_workspace(dm_plan *plan, void *dev, size_t bytes);
+
+/* Load a problem: stores sqrt(I) (in the spectrum layout of the kernels),
+ * copies P0 and O0, sets psi_jkl = P0_k * O0_l|window, freezes the absolute regularisers
+ * from P0/O0 (reading A8), uploads the tables and clears the error table.
+ * intensities DEV f32 [n_views][N][N] (>= 0, not validated on the device),
+ * probe0 DEV c64 [K][N][N], object0 DEV c64 [L][obj_h][obj_w].  Async on `stream`; the
+ * caller's buffers may be released once that stream work has completed.                */
+dm_status dm_set_data(dm_plan *plan, const float *intensities, const float *probe0,
+                      const float *object0, void *stream);
+
+/* Run n_iter >= 0 DM iterations (psi update eq. 3/4, object eq. 6, probe eq. 5, errors
+ * eq. 7), async on `stream`, no host synchronisation inside.  Appends n_iter error rows. */
+dm_status dm_iterate(dm_plan *plan, int n_iter, void *stream);
+
+/* Copy the current probe / object / psi to caller DEV buffers (async on `stream`).      */
+dm_status dm_get_probe(const dm_plan *plan, float *out_dev, void *stream);
+dm_status dm_get_object(const dm_plan *plan, float *out_dev, void *stream);
+dm_status dm_get_psi(const dm_plan *plan, float *out_dev, void *stream);
+
+/* Error table: row it = [eps_F, eps_psi, eps_P[0..K), eps_O[0..L)] as f64 (DESIGN.md
+ * reading A10; eq. (7)).  Copies min(rows, max_rows) rows to out_host (HOST) and SYNCS
+ * the device.                                                                          */
+dm_status dm_get_errors(const dm_plan *plan, double *out_host, int max_rows, int *rows_written);
+
+/* Parity hook (teacher forcing): overwrite probe / object / psi from DEV buffers; NULL =
+ * keep.  Does not touch sqrt(I), the frozen regularisers or the error table.           */
+dm_status dm_set_state(dm_plan *plan, const float *probe_dev, const float *object_dev,
+                       const float *psi_dev, void *stream);
+
+/* Integer tables of step S0 (HOST outputs, no CUDA call), compared bit-exactly with the
+ * oracle's.  Window table: int32 [n_views][3] = (y0, x0, y0*obj_w + x0).               */
+dm_status dm_get_window_table(const dm_plan *plan, int32_t *out_host);
+/* Coverage lists: for every tile_h x tile_w object tile (row-major), the ascending list of
+ * views whose window intersects it, as CSR.  Call once with tile_ptr_host = tile_views_host
+ * = NULL to get tile_h, tile_w and nnz; then with arrays of n_tiles+1 and nnz entries.   */
+dm_status dm_get_coverage(const dm_plan *plan, int *tile_h, int *tile_w, int32_t *tile_ptr_host,
+                          int32_t *tile_views_host, int64_t *nnz);
+
+/* The frozen absolute regularisers (alpha_obj, alpha_probe) computed by dm_set_data, as
+ * f64[2] to HOST.  SYNCS.                                                              */
+dm_status dm_get_alphas(const dm_plan *plan, double *out_host2);
+
+/* End-to-end entry with HOST buffers (what a beamline caller with data in host memory
+ * does): copies intensities / probe0 / object0 HOST->DEV into a staging
+ * area inside the workspace, runs dm_set_data + n_iter iterations, copies probe and object
+ * DEV->HOST, and SYNCS.  out_probe_host / out_object_host may be NULL.  Needs the
+ * workspace (which includes the staging area).                                          */
+dm_status dm_solve_host(dm_plan *plan, const float *intensities_host, const float *probe0_host,
+                        const float *object0_host, int n_iter, float *out_probe_host,
+                        float *out_object_host, void *stream);
+
+/* Which path dm_iterate runs for this plan: 1 staged, 2 fused (valid after dm_set_data);
+ * and how many kernels one iteration launches (the bench's gpu_launches claim).           */
+dm_status dm_plan_info(const dm_plan *plan, int *path, int *launches_per_iter);
+
+/* Test hook, HOST only, no CUDA call: runs the kernels' own FFT pass code (the same
+ * __host__ __device__ functions the kernels inline: radix butterflies, twiddle table,
+ * swizzled tile addressing, digit-reversal map) single-threaded on the host for one
+ * N x N frame and returns the spectrum in natural order.  in/out HOST c64 [N][N].       */
+dm_status dm_host_fft2(int N, const float *in_host, float *out_host, int inverse);
+
+const char *dm_status_string(dm_status s);
+const char *dm_last_error(const dm_plan *plan); /* plan may be NULL: last create error */
+void dm_plan_destroy(dm_plan *plan);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* DM_B200_H */

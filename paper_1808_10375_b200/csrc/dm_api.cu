@@ -1,0 +1,656 @@
+// dm_api.cu -- the C ABI of include/dm.h: host plan (integer tables, workspace carving),
+// launch orchestration of one DM iteration, getters.  No torch types, no exceptions.
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "../../include/dm.h"
+#include "dm_kernels.cuh"
+
+namespace {
+
+constexpr size_t ALIGN = 256;
+constexpr int ERR_ROWS_CAP = 16384;
+constexpr size_t SCRATCH_TARGET = 48u << 20;     // staged path: spectra of one chunk stay in L2
+constexpr int COLS_SW = 8;                        // staged path: spectrum columns per CTA
+
+thread_local std::string g_create_error;
+
+size_t align_up(size_t x) { return (x + ALIGN - 1) / ALIGN * ALIGN; }
+
+} // namespace
+
+struct dm_plan {
+    int N, n_views, K, L, M, H, W;
+    std::vector<int32_t> pos;            // (y0,x0)
+    std::vector<int32_t> tile_ptr, tile_views;
+    int nty, ntx;
+    std::vector<int32_t> rev;            // digit reversal of the FFT passes
+    std::vector<float> tw;               // N complex twiddles
+    double beta, a_obj, a_probe, eps_f;
+    int path_req, path;                  // requested / chosen (1 staged, 2 fused)
+    // probe reduction geometry
+    int prb_blocks, prb_chunks, prb_chunk_len, fin_blocks;
+    // staged geometry
+    int chunk_views;
+    // workspace
+    void *ws;
+    size_t ws_bytes, need_bytes;
+    float2 *psi, *Pbuf[2], *Obuf[2], *pnum, *scratch, *tw_d;
+    float *amp, *pden, *den_tmp, *alphas, *partA, *partB, *partP, *partO;
+    int2 *pos_d;
+    int *tile_ptr_d, *tile_views_d, *rev_d;
+    double *errors;
+    float *stage_I;
+    float2 *stage_P, *stage_O;
+    int curP, curO;
+    int nA, nB;                          // counts of (num,den) pairs in partA / partB (staged)
+    bool has_data;
+    int rows;
+    mutable std::string err;
+};
+
+namespace {
+
+dm_status fail(const dm_plan *p, dm_status s, const char *fmt, ...)
+{
+    char buf[512];
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(buf, sizeof buf, fmt, ap);
+    va_end(ap);
+    if (p) p->err = buf; else g_create_error = buf;
+    return s;
+}
+
+#define CU(call)                                                                              \
+    do {                                                                                      \
+        cudaError_t e_ = (call);                                                              \
+        if (e_ != cudaSuccess) return fail(plan, DM_ERR_CUDA, "%s: %s", #call, cudaGetErrorString(e_)); \
+    } while (0)
+
+template <int N> void fill_rev(std::vector<int32_t> &rev)
+{
+    rev.resize(N);
+    for (int p = 0; p < N; ++p) rev[p] = dmfft::digit_reverse<N>(p);
+}
+
+void build_tables(dm_plan *p)
+{
+    const int N = p->N, TH = OBJ_TH, TW = OBJ_TW;
+    p->nty = (p->H + TH - 1) / TH;
+    p->ntx = (p->W + TW - 1) / TW;
+    const int nt = p->nty * p->ntx;
+    std::vector<int32_t> cnt(nt + 1, 0);
+    for (int j = 0; j < p->n_views; ++j) {
+        const int y0 = p->pos[2 * j], x0 = p->pos[2 * j + 1];
+        for (int ty = y0 / TH; ty <= (y0 + N - 1) / TH; ++ty)
+            for (int tx = x0 / TW; tx <= (x0 + N - 1) / TW; ++tx) cnt[ty * p->ntx + tx + 1]++;
+    }
+    for (int t = 0; t < nt; ++t) cnt[t + 1] += cnt[t];
+    p->tile_ptr = cnt;
+    p->tile_views.assign((size_t)cnt[nt], 0);
+    std::vector<int32_t> fill(cnt.begin(), cnt.end() - 1);
+    for (int j = 0; j < p->n_views; ++j) {     // j ascending -> every list ascending
+        const int y0 = p->pos[2 * j], x0 = p->pos[2 * j + 1];
+        for (int ty = y0 / TH; ty <= (y0 + N - 1) / TH; ++ty)
+            for (int tx = x0 / TW; tx <= (x0 + N - 1) / TW; ++tx) p->tile_views[fill[ty * p->ntx + tx]++] = j;
+    }
+    switch (N) {
+    case 64: fill_rev<64>(p->rev); break;
+    case 128: fill_rev<128>(p->rev); break;
+    case 256: fill_rev<256>(p->rev); break;
+    default: fill_rev<512>(p->rev); break;
+    }
+    p->tw.resize(2 * (size_t)N);
+    for (int n = 0; n < N; ++n) {
+        const double ang = -2.0 * M_PI * (double)n / (double)N;
+        p->tw[2 * n] = (float)std::cos(ang);
+        p->tw[2 * n + 1] = (float)std::sin(ang);
+    }
+}
+
+void plan_geometry(dm_plan *p)
+{
+    const size_t NN = (size_t)p->N * p->N;
+    p->prb_blocks = (int)((NN / 2 + PRB_NT - 1) / PRB_NT);
+    int chunks = (148 * 16 + p->prb_blocks - 1) / p->prb_blocks;        // ~16 CTAs per SM in flight
+    if (chunks > p->n_views) chunks = p->n_views;
+    if (chunks < 1) chunks = 1;
+    p->prb_chunk_len = (p->n_views + chunks - 1) / chunks;
+    p->prb_chunks = (p->n_views + p->prb_chunk_len - 1) / p->prb_chunk_len;
+    p->fin_blocks = (int)((NN + 255) / 256);
+    const size_t per_view = (size_t)p->M * NN * sizeof(float2);
+    size_t cv = SCRATCH_TARGET / per_view;
+    if (cv < 1) cv = 1;
+    if (cv > (size_t)p->n_views) cv = p->n_views;
+    p->chunk_views = (int)cv;
+}
+
+// carve (or, with base == nullptr, just measure) the workspace
+size_t carve(dm_plan *p, unsigned char *base)
+{
+    size_t off = 0;
+    auto take = [&](size_t bytes) -> void * {
+        void *r = base ? base + off : nullptr;
+        off += align_up(bytes);
+        return r;
+    };
+    const size_t NN = (size_t)p->N * p->N, HW = (size_t)p->H * p->W;
+    const size_t MV = (size_t)p->n_views * p->M;
+    const int rows_tiles = p->N / (4096 / p->N);                         // row tiles per frame (staged)
+    p->nA = p->n_views * (p->N / COLS_SW);
+    p->nB = (int)(MV * rows_tiles);
+    p->psi = (float2 *)take(MV * NN * sizeof(float2));
+    p->amp = (float *)take((size_t)p->n_views * NN * sizeof(float));
+    for (int i = 0; i < 2; ++i) p->Pbuf[i] = (float2 *)take(p->K * NN * sizeof(float2));
+    for (int i = 0; i < 2; ++i) p->Obuf[i] = (float2 *)take(p->L * HW * sizeof(float2));
+    p->pnum = (float2 *)take((size_t)p->prb_chunks * p->K * NN * sizeof(float2));
+    p->pden = (float *)take((size_t)p->prb_chunks * NN * sizeof(float));
+    p->den_tmp = (float *)take((HW > NN ? HW : NN) * sizeof(float));
+    p->alphas = (float *)take(2 * sizeof(float));
+    const size_t nA = (size_t)p->nA * 2 > MV * 4 ? (size_t)p->nA * 2 : MV * 4;
+    p->partA = (float *)take(nA * sizeof(float));
+    p->partB = (float *)take((size_t)p->nB * 2 * sizeof(float));
+    p->partP = (float *)take((size_t)p->fin_blocks * p->K * 2 * sizeof(float));
+    p->partO = (float *)take((size_t)p->nty * p->ntx * p->L * 2 * sizeof(float));
+    p->pos_d = (int2 *)take((size_t)p->n_views * sizeof(int2));
+    p->tile_ptr_d = (int *)take(p->tile_ptr.size() * sizeof(int));
+    p->tile_views_d = (int *)take((p->tile_views.size() + 1) * sizeof(int));
+    p->rev_d = (int *)take(p->N * sizeof(int));
+    p->tw_d = (float2 *)take(p->N * sizeof(float2));
+    p->errors = (double *)take((size_t)ERR_ROWS_CAP * (2 + p->K + p->L) * sizeof(double));
+    p->scratch = (float2 *)take((size_t)p->chunk_views * p->M * NN * sizeof(float2));
+    p->stage_I = (float *)take((size_t)p->n_views * NN * sizeof(float));
+    p->stage_P = (float2 *)take(p->K * NN * sizeof(float2));
+    p->stage_O = (float2 *)take(p->L * HW * sizeof(float2));
+    return off;
+}
+
+PsiArgs psi_args(const dm_plan *p)
+{
+    PsiArgs a;
+    memset(&a, 0, sizeof a);
+    a.n_views = p->n_views; a.K = p->K; a.L = p->L; a.H = p->H; a.W = p->W;
+    a.pos = p->pos_d; a.P = p->Pbuf[p->curP]; a.O = p->Obuf[p->curO];
+    a.psi = p->psi; a.amp = p->amp; a.tw = p->tw_d;
+    a.beta = (float)p->beta; a.eps = (float)p->eps_f;
+    a.part = p->partA; a.part2 = p->partB; a.scratch = p->scratch;
+    return a;
+}
+
+template <int N, int NT> dm_status launch_fused(dm_plan *plan, cudaStream_t st)
+{
+    const size_t smem = (size_t)N * N * (sizeof(float2) + sizeof(float)) + N * sizeof(float2);
+    static bool attr_done = false;
+    if (!attr_done) {
+        CU(cudaFuncSetAttribute(fused_frame_kernel<N, NT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        attr_done = true;
+    }
+    PsiArgs a = psi_args(plan);
+    cudaLaunchConfig_t cfg;
+    memset(&cfg, 0, sizeof cfg);
+    cfg.gridDim = dim3((unsigned)(plan->n_views * plan->M));
+    cfg.blockDim = dim3(NT);
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = st;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeClusterDimension;
+    at[0].val.clusterDim.x = (unsigned)plan->M;
+    at[0].val.clusterDim.y = 1;
+    at[0].val.clusterDim.z = 1;
+    cfg.attrs = at;
+    cfg.numAttrs = 1;
+    CU(cudaLaunchKernelEx(&cfg, fused_frame_kernel<N, NT>, a));
+    return DM_OK;
+}
+
+template <int N> dm_status launch_staged(dm_plan *plan, cudaStream_t st)
+{
+    constexpr int ROWS = 4096 / N, NT = 256, SW = COLS_SW;
+    const size_t smem = (size_t)plan->M * N * SW * sizeof(float2);
+    static bool attr_done = false;
+    if (!attr_done) {
+        CU(cudaFuncSetAttribute(cols_mod_kernel<N, SW, NT>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
+        attr_done = true;
+    }
+    PsiArgs a = psi_args(plan);
+    for (int v0 = 0; v0 < plan->n_views; v0 += plan->chunk_views) {
+        const int nv = plan->n_views - v0 < plan->chunk_views ? plan->n_views - v0 : plan->chunk_views;
+        a.view0 = v0;
+        a.n_chunk = nv;
+        const unsigned row_tiles = (unsigned)(nv * plan->M * (N / ROWS));
+        rows_fwd_kernel<N, ROWS, NT><<<row_tiles, NT, 0, st>>>(a);
+        cols_mod_kernel<N, SW, NT><<<dim3(N / SW, nv), NT, smem, st>>>(a);
+        rows_inv_kernel<N, ROWS, NT><<<row_tiles, NT, 0, st>>>(a);
+    }
+    CU(cudaGetLastError());
+    return DM_OK;
+}
+
+dm_status launch_psi_update(dm_plan *plan, cudaStream_t st)
+{
+    if (plan->path == 2) {
+        if (plan->N == 64) return launch_fused<64, 256>(plan, st);
+        return launch_fused<128, 512>(plan, st);
+    }
+    switch (plan->N) {
+    case 64: return launch_staged<64>(plan, st);
+    case 128: return launch_staged<128>(plan, st);
+    case 256: return launch_staged<256>(plan, st);
+    default: return launch_staged<512>(plan, st);
+    }
+}
+
+dm_status launch_object(dm_plan *plan, cudaStream_t st, const float2 *P, const float2 *O_old, float2 *O_new,
+                        float *den_out)
+{
+    const int tiles = plan->nty * plan->ntx;
+#define OBJ_LAUNCH(LT)                                                                              \
+    object_gather_kernel<LT><<<tiles, OBJ_NT, 0, st>>>(plan->N, plan->K, plan->H, plan->W, plan->pos_d, \
+        plan->tile_ptr_d, plan->tile_views_d, P, plan->psi, O_old, O_new, plan->alphas, plan->partO, den_out)
+    switch (plan->L) {
+    case 1: OBJ_LAUNCH(1); break;
+    case 2: OBJ_LAUNCH(2); break;
+    case 3: OBJ_LAUNCH(3); break;
+    case 4: OBJ_LAUNCH(4); break;
+    case 5: OBJ_LAUNCH(5); break;
+    case 6: OBJ_LAUNCH(6); break;
+    case 7: OBJ_LAUNCH(7); break;
+    default: OBJ_LAUNCH(8); break;
+    }
+#undef OBJ_LAUNCH
+    CU(cudaGetLastError());
+    return DM_OK;
+}
+
+dm_status launch_probe(dm_plan *plan, cudaStream_t st, const float2 *O, const float2 *P_old, float2 *P_new,
+                       float *den_out)
+{
+    const dim3 grid((unsigned)plan->prb_blocks, (unsigned)plan->prb_chunks);
+#define PRB_LAUNCH(KT)                                                                              \
+    probe_partial_kernel<KT><<<grid, PRB_NT, 0, st>>>(plan->N, plan->L, plan->n_views, plan->prb_chunk_len, \
+        plan->H, plan->W, plan->pos_d, O, plan->psi, plan->pnum, plan->pden)
+    switch (plan->K) {
+    case 1: PRB_LAUNCH(1); break;
+    case 2: PRB_LAUNCH(2); break;
+    case 3: PRB_LAUNCH(3); break;
+    case 4: PRB_LAUNCH(4); break;
+    case 5: PRB_LAUNCH(5); break;
+    case 6: PRB_LAUNCH(6); break;
+    case 7: PRB_LAUNCH(7); break;
+    default: PRB_LAUNCH(8); break;
+    }
+#undef PRB_LAUNCH
+    probe_finalize_kernel<<<plan->fin_blocks, 256, 0, st>>>(plan->N, plan->K, plan->prb_chunks, plan->pnum, plan->pden,
+                                                            P_old, P_new, plan->alphas, plan->partP, den_out);
+    CU(cudaGetLastError());
+    return DM_OK;
+}
+
+dm_status check_ready(const dm_plan *plan, bool need_data)
+{
+    if (!plan) return DM_ERR_INVALID_ARG;
+    if (!plan->ws) return fail(plan, DM_ERR_WORKSPACE, "no workspace set");
+    if (need_data && !plan->has_data) return fail(plan, DM_ERR_NO_DATA, "dm_set_data has not been called");
+    return DM_OK;
+}
+
+} // namespace
+
+extern "C" {
+
+dm_status dm_plan_create(dm_plan **out, int N, int n_views, int K, int L, int obj_h, int obj_w,
+                         const int32_t *positions)
+{
+    if (!out) return fail(nullptr, DM_ERR_INVALID_ARG, "out is NULL");
+    *out = nullptr;
+    if (!positions) return fail(nullptr, DM_ERR_INVALID_ARG, "positions is NULL");
+    if (N <= 0 || n_views <= 0 || K <= 0 || L <= 0 || obj_h <= 0 || obj_w <= 0)
+        return fail(nullptr, DM_ERR_INVALID_ARG, "sizes must be positive");
+    if (N != 64 && N != 128 && N != 256 && N != 512)
+        return fail(nullptr, DM_ERR_UNSUPPORTED, "N = %d: supported frame edges are 64, 128, 256, 512", N);
+    if ((long long)K * L > 8) return fail(nullptr, DM_ERR_UNSUPPORTED, "K*L = %d > 8", K * L);
+    if (obj_w & 1) return fail(nullptr, DM_ERR_UNSUPPORTED, "obj_w = %d must be even", obj_w);
+    if ((long long)obj_h * obj_w > (1ll << 30) || (long long)n_views * K * L > (1ll << 24))
+        return fail(nullptr, DM_ERR_UNSUPPORTED, "problem too large for 32-bit indexing of tables");
+    for (int j = 0; j < n_views; ++j) {
+        const int y0 = positions[2 * j], x0 = positions[2 * j + 1];
+        if (y0 < 0 || x0 < 0 || (long long)y0 + N > obj_h || (long long)x0 + N > obj_w)
+            return fail(nullptr, DM_ERR_OUT_OF_BOUNDS, "view %d window (%d,%d)+%d leaves the %dx%d object", j, y0, x0, N,
+                        obj_h, obj_w);
+    }
+    dm_plan *p = new (std::nothrow) dm_plan();
+    if (!p) return fail(nullptr, DM_ERR_INVALID_ARG, "out of host memory");
+    p->N = N; p->n_views = n_views; p->K = K; p->L = L; p->M = K * L; p->H = obj_h; p->W = obj_w;
+    p->pos.assign(positions, positions + 2 * (size_t)n_views);
+    p->beta = 1.0; p->a_obj = 1e-3; p->a_probe = 1e-3; p->eps_f = 1e-30;
+    p->path_req = 0; p->path = 0;
+    p->ws = nullptr; p->ws_bytes = 0;
+    p->curP = p->curO = 0; p->has_data = false; p->rows = 0;
+    build_tables(p);
+    plan_geometry(p);
+    p->need_bytes = carve(p, nullptr);
+    *out = p;
+    return DM_OK;
+}
+
+dm_status dm_plan_set_param(dm_plan *plan, dm_param which, double v)
+{
+    if (!plan) return DM_ERR_INVALID_ARG;
+    if (plan->has_data) return fail(plan, DM_ERR_INVALID_ARG, "parameters must be set before dm_set_data");
+    if (!(v == v)) return fail(plan, DM_ERR_INVALID_ARG, "NaN parameter");
+    switch (which) {
+    case DM_PARAM_BETA: if (v < 0 || v > 1) break; plan->beta = v; return DM_OK;
+    case DM_PARAM_ALPHA_OBJ: if (v < 0) break; plan->a_obj = v; return DM_OK;
+    case DM_PARAM_ALPHA_PROBE: if (v < 0) break; plan->a_probe = v; return DM_OK;
+    case DM_PARAM_EPS_F: if (v < 0) break; plan->eps_f = v; return DM_OK;
+    case DM_PARAM_PATH: if (v != 0 && v != 1 && v != 2) break; plan->path_req = (int)v; return DM_OK;
+    default: return fail(plan, DM_ERR_INVALID_ARG, "unknown parameter %d", (int)which);
+    }
+    return fail(plan, DM_ERR_INVALID_ARG, "parameter %d: value %g out of range", (int)which, v);
+}
+
+dm_status dm_plan_workspace_bytes(const dm_plan *plan, size_t *bytes)
+{
+    if (!plan || !bytes) return DM_ERR_INVALID_ARG;
+    *bytes = plan->need_bytes;
+    return DM_OK;
+}
+
+dm_status dm_plan_set_workspace(dm_plan *plan, void *dev, size_t bytes)
+{
+    if (!plan) return DM_ERR_INVALID_ARG;
+    if (!dev) return fail(plan, DM_ERR_INVALID_ARG, "workspace pointer is NULL");
+    if ((uintptr_t)dev % ALIGN) return fail(plan, DM_ERR_WORKSPACE, "workspace must be 256-byte aligned");
+    if (bytes < plan->need_bytes)
+        return fail(plan, DM_ERR_WORKSPACE, "workspace of %zu bytes < %zu needed", bytes, plan->need_bytes);
+    plan->ws = dev;
+    plan->ws_bytes = bytes;
+    carve(plan, (unsigned char *)dev);
+    plan->has_data = false;
+    return DM_OK;
+}
+
+dm_status dm_set_data(dm_plan *plan, const float *intensities, const float *probe0, const float *object0, void *stream)
+{
+    dm_status s = check_ready(plan, false);
+    if (s != DM_OK) return s;
+    if (!intensities || !probe0 || !object0) return fail(plan, DM_ERR_INVALID_ARG, "NULL data pointer");
+    int path = plan->path_req;
+    if (path == 0) path = (plan->N <= 128) ? 2 : 1;
+    if (path == 2 && plan->N > 128)
+        return fail(plan, DM_ERR_UNSUPPORTED, "fused per-frame path needs N <= 128 (N = %d)", plan->N);
+    plan->path = path;
+    cudaStream_t st = (cudaStream_t)stream;
+    const size_t NN = (size_t)plan->N * plan->N, HW = (size_t)plan->H * plan->W;
+    CU(cudaMemcpyAsync(plan->pos_d, plan->pos.data(), plan->pos.size() * sizeof(int32_t), cudaMemcpyHostToDevice, st));
+    CU(cudaMemcpyAsync(plan->tile_ptr_d, plan->tile_ptr.data(), plan->tile_ptr.size() * sizeof(int32_t), cudaMemcpyHostToDevice, st));
+    if (!plan->tile_views.empty())
+        CU(cudaMemcpyAsync(plan->tile_views_d, plan->tile_views.data(), plan->tile_views.size() * sizeof(int32_t), cudaMemcpyHostToDevice, st));
+    CU(cudaMemcpyAsync(plan->rev_d, plan->rev.data(), plan->rev.size() * sizeof(int32_t), cudaMemcpyHostToDevice, st));
+    CU(cudaMemcpyAsync(plan->tw_d, plan->tw.data(), plan->tw.size() * sizeof(float), cudaMemcpyHostToDevice, st));
+    plan->curP = plan->curO = 0;
+    CU(cudaMemcpyAsync(plan->Pbuf[0], probe0, plan->K * NN * sizeof(float2), cudaMemcpyDeviceToDevice, st));
+    CU(cudaMemcpyAsync(plan->Obuf[0], object0, plan->L * HW * sizeof(float2), cudaMemcpyDeviceToDevice, st));
+    CU(cudaMemsetAsync(plan->alphas, 0, 2 * sizeof(float), st));
+    const size_t total = (size_t)plan->n_views * NN;
+    amp_permute_kernel<<<148 * 8, 256, 0, st>>>(plan->N, intensities, plan->rev_d, plan->amp, total);
+    psi_init_kernel<<<dim3((unsigned)((NN + 1023) / 1024), (unsigned)(plan->n_views * plan->M)), 256, 0, st>>>(
+        plan->N, plan->K, plan->L, plan->H, plan->W, plan->pos_d, plan->Pbuf[0], plan->Obuf[0], plan->psi);
+    CU(cudaGetLastError());
+    // frozen regularisers (reading A8): alpha_O = a_O max_r den_O(P0), alpha_P = a_P max_r den_P(O0);
+    // the two update kernels run once with alpha = 0 into the spare buffers just to produce den.
+    s = launch_object(plan, st, plan->Pbuf[0], plan->Obuf[0], plan->Obuf[1], plan->den_tmp);
+    if (s != DM_OK) return s;
+    max_scale_kernel<<<1, 1024, 0, st>>>(plan->den_tmp, HW, (float)plan->a_obj, plan->alphas);
+    s = launch_probe(plan, st, plan->Obuf[0], plan->Pbuf[0], plan->Pbuf[1], plan->den_tmp);
+    if (s != DM_OK) return s;
+    max_scale_kernel<<<1, 1024, 0, st>>>(plan->den_tmp, NN, (float)plan->a_probe, plan->alphas + 1);
+    CU(cudaGetLastError());
+    plan->has_data = true;
+    plan->rows = 0;
+    return DM_OK;
+}
+
+dm_status dm_iterate(dm_plan *plan, int n_iter, void *stream)
+{
+    dm_status s = check_ready(plan, true);
+    if (s != DM_OK) return s;
+    if (n_iter < 0) return fail(plan, DM_ERR_INVALID_ARG, "n_iter = %d < 0", n_iter);
+    if (plan->rows + n_iter > ERR_ROWS_CAP)
+        return fail(plan, DM_ERR_WORKSPACE, "error table holds %d rows; call dm_set_data to reset", ERR_ROWS_CAP);
+    cudaStream_t st = (cudaStream_t)stream;
+    const int ncol = 2 + plan->K + plan->L;
+    for (int it = 0; it < n_iter; ++it) {
+        s = launch_psi_update(plan, st);                                           // S1-S6
+        if (s != DM_OK) return s;
+        const int nO = 1 - plan->curO, nP = 1 - plan->curP;
+        s = launch_object(plan, st, plan->Pbuf[plan->curP], plan->Obuf[plan->curO], plan->Obuf[nO], nullptr);   // S7
+        if (s != DM_OK) return s;
+        s = launch_probe(plan, st, plan->Obuf[nO], plan->Pbuf[plan->curP], plan->Pbuf[nP], nullptr);            // S8
+        if (s != DM_OK) return s;
+        ErrArgs e;                                                                   // S9
+        if (plan->path == 2) {
+            e.pF = plan->partA;     e.nF = plan->n_views * plan->M; e.sF = 4;
+            e.pS = plan->partA + 2; e.nS = plan->n_views * plan->M; e.sS = 4;
+        } else {
+            e.pF = plan->partA; e.nF = plan->nA; e.sF = 2;
+            e.pS = plan->partB; e.nS = plan->nB; e.sS = 2;
+        }
+        e.pP = plan->partP; e.nP = plan->fin_blocks;
+        e.pO = plan->partO; e.nO = plan->nty * plan->ntx;
+        e.K = plan->K; e.L = plan->L;
+        e.row = plan->errors + (size_t)plan->rows * ncol;
+        error_finalize_kernel<<<ncol, 256, 0, st>>>(e);
+        CU(cudaGetLastError());
+        plan->curO = nO;
+        plan->curP = nP;
+        plan->rows++;
+    }
+    return DM_OK;
+}
+
+dm_status dm_get_probe(const dm_plan *plan, float *out_dev, void *stream)
+{
+    dm_status s = check_ready(plan, true);
+    if (s != DM_OK) return s;
+    if (!out_dev) return fail(plan, DM_ERR_INVALID_ARG, "NULL output");
+    CU(cudaMemcpyAsync(out_dev, plan->Pbuf[plan->curP], (size_t)plan->K * plan->N * plan->N * sizeof(float2),
+                       cudaMemcpyDeviceToDevice, (cudaStream_t)stream));
+    return DM_OK;
+}
+
+dm_status dm_get_object(const dm_plan *plan, float *out_dev, void *stream)
+{
+    dm_status s = check_ready(plan, true);
+    if (s != DM_OK) return s;
+    if (!out_dev) return fail(plan, DM_ERR_INVALID_ARG, "NULL output");
+    CU(cudaMemcpyAsync(out_dev, plan->Obuf[plan->curO], (size_t)plan->L * plan->H * plan->W * sizeof(float2),
+                       cudaMemcpyDeviceToDevice, (cudaStream_t)stream));
+    return DM_OK;
+}
+
+dm_status dm_get_psi(const dm_plan *plan, float *out_dev, void *stream)
+{
+    dm_status s = check_ready(plan, true);
+    if (s != DM_OK) return s;
+    if (!out_dev) return fail(plan, DM_ERR_INVALID_ARG, "NULL output");
+    CU(cudaMemcpyAsync(out_dev, plan->psi, (size_t)plan->n_views * plan->M * plan->N * plan->N * sizeof(float2),
+                       cudaMemcpyDeviceToDevice, (cudaStream_t)stream));
+    return DM_OK;
+}
+
+dm_status dm_get_errors(const dm_plan *plan, double *out_host, int max_rows, int *rows_written)
+{
+    dm_status s = check_ready(plan, true);
+    if (s != DM_OK) return s;
+    if (!out_host || !rows_written || max_rows < 0) return fail(plan, DM_ERR_INVALID_ARG, "bad output arguments");
+    CU(cudaDeviceSynchronize());
+    const int n = plan->rows < max_rows ? plan->rows : max_rows;
+    if (n > 0) CU(cudaMemcpy(out_host, plan->errors, (size_t)n * (2 + plan->K + plan->L) * sizeof(double), cudaMemcpyDeviceToHost));
+    *rows_written = n;
+    return DM_OK;
+}
+
+dm_status dm_set_state(dm_plan *plan, const float *probe_dev, const float *object_dev, const float *psi_dev, void *stream)
+{
+    dm_status s = check_ready(plan, true);
+    if (s != DM_OK) return s;
+    cudaStream_t st = (cudaStream_t)stream;
+    const size_t NN = (size_t)plan->N * plan->N, HW = (size_t)plan->H * plan->W;
+    if (probe_dev) CU(cudaMemcpyAsync(plan->Pbuf[plan->curP], probe_dev, plan->K * NN * sizeof(float2), cudaMemcpyDeviceToDevice, st));
+    if (object_dev) CU(cudaMemcpyAsync(plan->Obuf[plan->curO], object_dev, plan->L * HW * sizeof(float2), cudaMemcpyDeviceToDevice, st));
+    if (psi_dev) CU(cudaMemcpyAsync(plan->psi, psi_dev, (size_t)plan->n_views * plan->M * NN * sizeof(float2), cudaMemcpyDeviceToDevice, st));
+    return DM_OK;
+}
+
+dm_status dm_get_window_table(const dm_plan *plan, int32_t *out_host)
+{
+    if (!plan || !out_host) return DM_ERR_INVALID_ARG;
+    for (int j = 0; j < plan->n_views; ++j) {
+        out_host[3 * j] = plan->pos[2 * j];
+        out_host[3 * j + 1] = plan->pos[2 * j + 1];
+        out_host[3 * j + 2] = plan->pos[2 * j] * plan->W + plan->pos[2 * j + 1];
+    }
+    return DM_OK;
+}
+
+dm_status dm_get_coverage(const dm_plan *plan, int *tile_h, int *tile_w, int32_t *tile_ptr_host,
+                          int32_t *tile_views_host, int64_t *nnz)
+{
+    if (!plan || !tile_h || !tile_w || !nnz) return DM_ERR_INVALID_ARG;
+    *tile_h = OBJ_TH;
+    *tile_w = OBJ_TW;
+    *nnz = (int64_t)plan->tile_views.size();
+    if (tile_ptr_host) memcpy(tile_ptr_host, plan->tile_ptr.data(), plan->tile_ptr.size() * sizeof(int32_t));
+    if (tile_views_host && !plan->tile_views.empty())
+        memcpy(tile_views_host, plan->tile_views.data(), plan->tile_views.size() * sizeof(int32_t));
+    return DM_OK;
+}
+
+dm_status dm_get_alphas(const dm_plan *plan, double *out_host2)
+{
+    dm_status s = check_ready(plan, true);
+    if (s != DM_OK) return s;
+    if (!out_host2) return fail(plan, DM_ERR_INVALID_ARG, "NULL output");
+    float a[2];
+    CU(cudaDeviceSynchronize());
+    CU(cudaMemcpy(a, plan->alphas, sizeof a, cudaMemcpyDeviceToHost));
+    out_host2[0] = a[0];
+    out_host2[1] = a[1];
+    return DM_OK;
+}
+
+dm_status dm_solve_host(dm_plan *plan, const float *intensities_host, const float *probe0_host,
+                        const float *object0_host, int n_iter, float *out_probe_host, float *out_object_host,
+                        void *stream)
+{
+    dm_status s = check_ready(plan, false);
+    if (s != DM_OK) return s;
+    if (!intensities_host || !probe0_host || !object0_host) return fail(plan, DM_ERR_INVALID_ARG, "NULL data pointer");
+    cudaStream_t st = (cudaStream_t)stream;
+    const size_t NN = (size_t)plan->N * plan->N, HW = (size_t)plan->H * plan->W;
+    CU(cudaMemcpyAsync(plan->stage_I, intensities_host, (size_t)plan->n_views * NN * sizeof(float), cudaMemcpyHostToDevice, st));
+    CU(cudaMemcpyAsync(plan->stage_P, probe0_host, plan->K * NN * sizeof(float2), cudaMemcpyHostToDevice, st));
+    CU(cudaMemcpyAsync(plan->stage_O, object0_host, plan->L * HW * sizeof(float2), cudaMemcpyHostToDevice, st));
+    plan->has_data = false;
+    s = dm_set_data(plan, plan->stage_I, (const float *)plan->stage_P, (const float *)plan->stage_O, stream);
+    if (s != DM_OK) return s;
+    s = dm_iterate(plan, n_iter, stream);
+    if (s != DM_OK) return s;
+    if (out_probe_host)
+        CU(cudaMemcpyAsync(out_probe_host, plan->Pbuf[plan->curP], plan->K * NN * sizeof(float2), cudaMemcpyDeviceToHost, st));
+    if (out_object_host)
+        CU(cudaMemcpyAsync(out_object_host, plan->Obuf[plan->curO], plan->L * HW * sizeof(float2), cudaMemcpyDeviceToHost, st));
+    CU(cudaStreamSynchronize(st));
+    return DM_OK;
+}
+
+dm_status dm_plan_info(const dm_plan *plan, int *path, int *launches_per_iter)
+{
+    if (!plan) return DM_ERR_INVALID_ARG;
+    int p = plan->path ? plan->path : (plan->path_req ? plan->path_req : (plan->N <= 128 ? 2 : 1));
+    if (path) *path = p;
+    if (launches_per_iter) {
+        const int chunks = (plan->n_views + plan->chunk_views - 1) / plan->chunk_views;
+        *launches_per_iter = (p == 2 ? 1 : 3 * chunks) + 4;
+    }
+    return DM_OK;
+}
+
+} // extern "C"
+
+namespace {
+struct NoSync { __host__ __device__ void operator()() const {} };
+template <int N> void host_fft2(const float *in, float *out, int inverse)
+{
+    std::vector<float2> tile((size_t)N * N), tw(N);
+    for (int n = 0; n < N; ++n) {
+        const double ang = -2.0 * M_PI * (double)n / (double)N;
+        tw[n] = make_float2((float)std::cos(ang), (float)std::sin(ang));
+    }
+    std::vector<int32_t> rev;
+    fill_rev<N>(rev);
+    const float2 *src = reinterpret_cast<const float2 *>(in);
+    float2 *dst = reinterpret_cast<float2 *>(out);
+    if (!inverse) {
+        for (int e = 0; e < N * N; ++e) tile[swz(e)] = src[e];
+        // emulate NT threads one after the other: butterflies of one pass touch disjoint elements
+        for (int t = 0; t < 64; ++t) tile_pass<N, Radix<N>::R1, N, false, false, N, N>(tile.data(), tw.data(), t, 64);
+        for (int t = 0; t < 64; ++t) tile_pass<N, Radix<N>::R2, N / Radix<N>::R1, false, false, N, N>(tile.data(), tw.data(), t, 64);
+        if (Radix<N>::R3 > 1)
+            for (int t = 0; t < 64; ++t) tile_pass<N, (Radix<N>::R3 > 1 ? Radix<N>::R3 : 2), (Radix<N>::R3 > 1 ? N / (Radix<N>::R1 * Radix<N>::R2) : 2), false, false, N, N>(tile.data(), tw.data(), t, 64);
+        axis_fft<N, false, true, N, N>(tile.data(), tw.data(), 0, 1, NoSync());
+        for (int py = 0; py < N; ++py)
+            for (int px = 0; px < N; ++px) dst[(size_t)rev[py] * N + rev[px]] = tile[swz(py * N + px)];
+    } else {
+        // input is a natural-order spectrum: place it in the kernels' permuted layout first
+        for (int py = 0; py < N; ++py)
+            for (int px = 0; px < N; ++px) tile[swz(py * N + px)] = src[(size_t)rev[py] * N + rev[px]];
+        axis_fft<N, true, true, N, N>(tile.data(), tw.data(), 0, 1, NoSync());
+        axis_fft<N, true, false, N, N>(tile.data(), tw.data(), 0, 1, NoSync());
+        const float s = 1.f / ((float)N * (float)N);
+        for (int e = 0; e < N * N; ++e) dst[e] = make_float2(tile[swz(e)].x * s, tile[swz(e)].y * s);
+    }
+}
+} // namespace
+
+extern "C" {
+
+dm_status dm_host_fft2(int N, const float *in_host, float *out_host, int inverse)
+{
+    if (!in_host || !out_host) return DM_ERR_INVALID_ARG;
+    switch (N) {
+    case 64: host_fft2<64>(in_host, out_host, inverse); break;
+    case 128: host_fft2<128>(in_host, out_host, inverse); break;
+    case 256: host_fft2<256>(in_host, out_host, inverse); break;
+    case 512: host_fft2<512>(in_host, out_host, inverse); break;
+    default: return DM_ERR_UNSUPPORTED;
+    }
+    return DM_OK;
+}
+
+const char *dm_status_string(dm_status s)
+{
+    switch (s) {
+    case DM_OK: return "DM_OK";
+    case DM_ERR_INVALID_ARG: return "DM_ERR_INVALID_ARG";
+    case DM_ERR_OUT_OF_BOUNDS: return "DM_ERR_OUT_OF_BOUNDS";
+    case DM_ERR_UNSUPPORTED: return "DM_ERR_UNSUPPORTED";
+    case DM_ERR_NO_DATA: return "DM_ERR_NO_DATA";
+    case DM_ERR_WORKSPACE: return "DM_ERR_WORKSPACE";
+    case DM_ERR_CUDA: return "DM_ERR_CUDA";
+    }
+    return "DM_ERR_?";
+}
+
+const char *dm_last_error(const dm_plan *plan) { return plan ? plan->err.c_str() : g_create_error.c_str(); }
+
+void dm_plan_destroy(dm_plan *plan) { delete plan; }
+
+} // extern "C"
