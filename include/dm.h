@@ -133,6 +133,14 @@ dm_status dm_solve_host(dm_plan *plan, const float *intensities_host, const floa
  * and how many kernels one iteration launches (the bench's gpu_launches claim).           */
 dm_status dm_plan_info(const dm_plan *plan, int *path, int *launches_per_iter);
 
+/* Per-phase device timing (measurement aid of bench.py; off by default).  When on, dm_iterate
+ * records CUDA events on `stream` around the four phases of every iteration (psi update S1-S6,
+ * object S7, probe S8, error row S9), for at most 4096 iterations between two reads.
+ * dm_get_phase_ms SYNCS, writes the summed milliseconds per phase to out_ms4 (HOST f32[4]) and
+ * the number of iterations they cover to *iters, and resets the accumulation.            */
+dm_status dm_plan_set_profiling(dm_plan *plan, int on);
+dm_status dm_get_phase_ms(dm_plan *plan, float *out_ms4, int *iters);
+
 /* Test hook, HOST only, no CUDA call: runs the kernels' own FFT pass code (the same
  * __host__ __device__ functions the kernels inline: radix butterflies, twiddle table,
  * swizzled tile addressing, digit-reversal map) single-threaded on the host for one

@@ -17,6 +17,7 @@ constexpr size_t ALIGN = 256;
 constexpr int ERR_ROWS_CAP = 16384;
 constexpr size_t SCRATCH_TARGET = 48u << 20;     // staged path: spectra of one chunk stay in L2
 constexpr int COLS_SW = 8;                        // staged path: spectrum columns per CTA
+constexpr int PROF_MAX_ITERS = 4096;
 
 thread_local std::string g_create_error;
 
@@ -51,6 +52,10 @@ struct dm_plan {
     int nA, nB;                          // counts of (num,den) pairs in partA / partB (staged)
     bool has_data;
     int rows;
+    // optional per-phase timing (dm_plan_set_profiling)
+    bool profiling;
+    std::vector<cudaEvent_t> ev;         // 5 events per profiled iteration
+    int ev_iters;
     mutable std::string err;
 };
 
@@ -332,6 +337,7 @@ dm_status dm_plan_create(dm_plan **out, int N, int n_views, int K, int L, int ob
     p->path_req = 0; p->path = 0;
     p->ws = nullptr; p->ws_bytes = 0;
     p->curP = p->curO = 0; p->has_data = false; p->rows = 0;
+    p->profiling = false; p->ev_iters = 0;
     build_tables(p);
     plan_geometry(p);
     p->need_bytes = carve(p, nullptr);
@@ -427,13 +433,26 @@ dm_status dm_iterate(dm_plan *plan, int n_iter, void *stream)
     cudaStream_t st = (cudaStream_t)stream;
     const int ncol = 2 + plan->K + plan->L;
     for (int it = 0; it < n_iter; ++it) {
+        cudaEvent_t *ev = nullptr;
+        if (plan->profiling && plan->ev_iters < PROF_MAX_ITERS) {
+            while ((int)plan->ev.size() < 5 * (plan->ev_iters + 1)) {
+                cudaEvent_t e;
+                CU(cudaEventCreate(&e));
+                plan->ev.push_back(e);
+            }
+            ev = plan->ev.data() + 5 * plan->ev_iters++;
+        }
+        if (ev) CU(cudaEventRecord(ev[0], st));
         s = launch_psi_update(plan, st);                                           // S1-S6
         if (s != DM_OK) return s;
+        if (ev) CU(cudaEventRecord(ev[1], st));
         const int nO = 1 - plan->curO, nP = 1 - plan->curP;
         s = launch_object(plan, st, plan->Pbuf[plan->curP], plan->Obuf[plan->curO], plan->Obuf[nO], nullptr);   // S7
         if (s != DM_OK) return s;
+        if (ev) CU(cudaEventRecord(ev[2], st));
         s = launch_probe(plan, st, plan->Obuf[nO], plan->Pbuf[plan->curP], plan->Pbuf[nP], nullptr);            // S8
         if (s != DM_OK) return s;
+        if (ev) CU(cudaEventRecord(ev[3], st));
         ErrArgs e;                                                                   // S9
         if (plan->path == 2) {
             e.pF = plan->partA;     e.nF = plan->n_views * plan->M; e.sF = 4;
@@ -448,6 +467,7 @@ dm_status dm_iterate(dm_plan *plan, int n_iter, void *stream)
         e.row = plan->errors + (size_t)plan->rows * ncol;
         error_finalize_kernel<<<ncol, 256, 0, st>>>(e);
         CU(cudaGetLastError());
+        if (ev) CU(cudaEventRecord(ev[4], st));
         plan->curO = nO;
         plan->curP = nP;
         plan->rows++;
@@ -571,6 +591,31 @@ dm_status dm_solve_host(dm_plan *plan, const float *intensities_host, const floa
     return DM_OK;
 }
 
+dm_status dm_plan_set_profiling(dm_plan *plan, int on)
+{
+    if (!plan) return DM_ERR_INVALID_ARG;
+    plan->profiling = on != 0;
+    plan->ev_iters = 0;
+    return DM_OK;
+}
+
+dm_status dm_get_phase_ms(dm_plan *plan, float *out_ms4, int *iters)
+{
+    if (!plan || !out_ms4 || !iters) return DM_ERR_INVALID_ARG;
+    CU(cudaDeviceSynchronize());
+    double acc[4] = {0, 0, 0, 0};
+    for (int i = 0; i < plan->ev_iters; ++i)
+        for (int ph = 0; ph < 4; ++ph) {
+            float ms = 0.f;
+            CU(cudaEventElapsedTime(&ms, plan->ev[5 * i + ph], plan->ev[5 * i + ph + 1]));
+            acc[ph] += ms;
+        }
+    for (int ph = 0; ph < 4; ++ph) out_ms4[ph] = (float)acc[ph];
+    *iters = plan->ev_iters;
+    plan->ev_iters = 0;
+    return DM_OK;
+}
+
 dm_status dm_plan_info(const dm_plan *plan, int *path, int *launches_per_iter)
 {
     if (!plan) return DM_ERR_INVALID_ARG;
@@ -651,6 +696,11 @@ const char *dm_status_string(dm_status s)
 
 const char *dm_last_error(const dm_plan *plan) { return plan ? plan->err.c_str() : g_create_error.c_str(); }
 
-void dm_plan_destroy(dm_plan *plan) { delete plan; }
+void dm_plan_destroy(dm_plan *plan)
+{
+    if (!plan) return;
+    for (cudaEvent_t e : plan->ev) cudaEventDestroy(e);
+    delete plan;
+}
 
 } // extern "C"

@@ -24,7 +24,7 @@ SYMBOLS = (
     "dm_plan_create", "dm_plan_set_param", "dm_plan_workspace_bytes", "dm_plan_set_workspace",
     "dm_set_data", "dm_iterate", "dm_get_probe", "dm_get_object", "dm_get_psi", "dm_get_errors",
     "dm_set_state", "dm_get_window_table", "dm_get_coverage", "dm_get_alphas", "dm_solve_host",
-    "dm_plan_info", "dm_host_fft2", "dm_status_string", "dm_last_error", "dm_plan_destroy",
+    "dm_plan_info", "dm_plan_set_profiling", "dm_get_phase_ms", "dm_host_fft2", "dm_status_string", "dm_last_error", "dm_plan_destroy",
 )
 
 _vp, _int, _dbl = C.c_void_p, C.c_int, C.c_double
@@ -61,6 +61,8 @@ def lib() -> C.CDLL:
         L.dm_get_alphas.argtypes = [_vp, _vp]
         L.dm_solve_host.argtypes = [_vp, _vp, _vp, _vp, _int, _vp, _vp, _vp]
         L.dm_plan_info.argtypes = [_vp, C.POINTER(_int), C.POINTER(_int)]
+        L.dm_plan_set_profiling.argtypes = [_vp, _int]
+        L.dm_get_phase_ms.argtypes = [_vp, _vp, C.POINTER(_int)]
         L.dm_host_fft2.argtypes = [_int, _vp, _vp, _int]
         L.dm_status_string.argtypes = [_int]
         L.dm_status_string.restype = C.c_char_p
@@ -201,6 +203,16 @@ class DMPlan:
         p, n = _int(), _int()
         self._check(self._lib.dm_plan_info(self._h, C.byref(p), C.byref(n)))
         return {"path": p.value, "launches_per_iter": n.value}
+
+    def set_profiling(self, on=True):
+        self._check(self._lib.dm_plan_set_profiling(self._h, int(bool(on))))
+
+    def phase_ms(self):
+        """Summed device milliseconds of (psi update, object, probe, errors) and the iteration count."""
+        out = np.zeros(4, np.float32)
+        n = _int()
+        self._check(self._lib.dm_get_phase_ms(self._h, _np_ptr(out), C.byref(n)))
+        return out.astype(np.float64), n.value
 
     # -- integer tables (host) ----------------------------------------------------------
     def window_table(self) -> np.ndarray:

@@ -1,0 +1,175 @@
+"""GPU parity: the CUDA path (through the C ABI) against the FP64 oracle, element by element,
+on the same seeded complex64/float32 inputs (SURVEY.md §8(c) protocol P1-P4).
+
+Tolerances (BASELINE.json north_star): bit-exact tables; relative L2 <= 1e-5 on psi, P, O after
+one iteration from an identical state; long free runs are reported against 1e-3 with the
+oracle's own FP32 build as the yardstick."""
+import numpy as np
+import pytest
+
+import oracle
+from paper_1808_10375_b200 import synth
+
+pytestmark = pytest.mark.gpu
+
+ONE_STEP_TOL = 1e-5
+
+
+@pytest.fixture(scope="module")
+def dm():
+    import torch
+    assert torch.cuda.is_available(), "the -m gpu tests need a CUDA device"
+    from paper_1808_10375_b200 import dm as _dm
+    _dm.lib()          # raises if the CUDA extension is missing: no fallback
+    return _dm
+
+
+def _t(a):
+    import torch
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def make_pair(dm, pr, **params):
+    c = pr.cfg
+    g = dm.DMPlan(c.N, c.n_views, c.K, c.L, c.obj_h, c.obj_w, pr.positions, **params).alloc_workspace()
+    g.set_data(_t(pr.intensities), _t(pr.probe0), _t(pr.object0))
+    o = oracle.OracleDM(c.N, c.K, c.L, c.obj_h, c.obj_w, pr.positions,
+                        **{k: v for k, v in params.items() if k != "path"})
+    o.set_data(pr.intensities, pr.probe0, pr.object0)
+    return g, o
+
+
+def compare_state(g, o, tol, what=""):
+    r = {"psi": synth.rel_l2(g.psi().cpu().numpy(), o.psi()),
+         "P": synth.rel_l2(g.probe().cpu().numpy(), o.probe()),
+         "O": synth.rel_l2(g.object().cpu().numpy(), o.object())}
+    for k, v in r.items():
+        assert v <= tol, f"{what} {k}: rel L2 {v:.3e} > {tol:g}  ({r})"
+    return r
+
+
+# (config index, raster ny, nx) : sizes the oracle finishes in seconds, several tiles + ragged tails
+SMALL = [(0, 10, 10), (1, 6, 5), (2, 5, 7), (3, 3, 3), (4, 2, 2)]
+
+
+@pytest.mark.parametrize("cfg_i,ny,nx", SMALL)
+@pytest.mark.parametrize("path", [0, 1])
+def test_one_iteration_parity(dm, cfg_i, ny, nx, path):
+    """P2 at t = 0: set_data state (psi = P0*O0, alphas), then one full iteration."""
+    pr = synth.make_problem(synth.CONFIGS[cfg_i].scaled(ny, nx))
+    g, o = make_pair(dm, pr, path=path)
+    compare_state(g, o, 1e-6, "t=0")                         # psi init is one complex multiply
+    ag, ao = g.alphas, o.alphas
+    assert abs(ag[0] - ao[0]) <= 1e-5 * ao[0] and abs(ag[1] - ao[1]) <= 1e-5 * ao[1]
+    g.iterate(1)
+    o.iterate(1)
+    compare_state(g, o, ONE_STEP_TOL, f"cfg{cfg_i} path{path} it1")
+    eg, eo = g.errors(), o.errors()
+    assert eg.shape == eo.shape == (1, 2 + pr.cfg.K + pr.cfg.L)
+    assert np.abs(eg - eo).max() <= 1e-5 * max(1.0, np.abs(eo).max())
+    g.close(); o.close()
+
+
+@pytest.mark.parametrize("cfg_i,ny,nx", [(0, 10, 10), (1, 6, 5)])
+@pytest.mark.parametrize("beta,a", [(0.8, 1e-3), (1.0, 0.0)])
+def test_one_iteration_parity_beta_and_literal_quotient(dm, cfg_i, ny, nx, beta, a):
+    """Readings A1 (beta = 0.8, the paper's usual value) and A8 (a = 0: the paper's literal
+    eqs. (5),(6)) must pass the same one-step bar."""
+    pr = synth.make_problem(synth.CONFIGS[cfg_i].scaled(ny, nx))
+    g, o = make_pair(dm, pr, beta=beta, alpha_obj=a, alpha_probe=a)
+    g.iterate(1)
+    o.iterate(1)
+    compare_state(g, o, ONE_STEP_TOL, f"beta={beta} a={a}")
+    g.close(); o.close()
+
+
+@pytest.mark.parametrize("cfg_i,ny,nx,n_iter", [(0, 10, 10, 50), (1, 6, 5, 30)])
+def test_teacher_forced_steps_and_short_free_runs(dm, cfg_i, ny, nx, n_iter):
+    """P2 teacher-forced along the oracle trajectory + P3 short free runs from checkpoints."""
+    pr = synth.make_problem(synth.CONFIGS[cfg_i].scaled(ny, nx))
+    g, o = make_pair(dm, pr)
+    marks = sorted({1, 5, 10, 25, n_iter - 1} & set(range(1, n_iter)))
+    t = 0
+    for m in marks:
+        o.iterate(m - t)
+        t = m
+        P, O, psi = o.probe(), o.object(), o.psi()
+        # identical complex64 state on both sides (A20): cast once, hand the cast values to both
+        P32, O32, psi32 = (x.astype(np.complex64) for x in (P, O, psi))
+        o2 = oracle.OracleDM(pr.cfg.N, pr.cfg.K, pr.cfg.L, pr.cfg.obj_h, pr.cfg.obj_w, pr.positions)
+        o2.set_data(pr.intensities, pr.probe0, pr.object0)        # amp + frozen alphas
+        o2.set_state(P32, O32, psi32)
+        g.set_state(_t(P32), _t(O32), _t(psi32))
+        g.iterate(1)
+        o2.iterate(1)
+        compare_state(g, o2, ONE_STEP_TOL, f"teacher-forced t={m}")
+        g.iterate(4)
+        o2.iterate(4)
+        compare_state(g, o2, 2e-4, f"5-step free run from t={m}")
+        o2.close()
+    g.close(); o.close()
+
+
+def test_free_run_config0_vs_fp64_and_fp32_yardstick(dm):
+    """P4: 50 free-running iterations of config 0.  The eps_F curve must meet the 1e-3 bar;
+    P and O are checked against max(1e-3, 2 x the oracle's own FP32-vs-FP64 divergence)
+    (the DM transient amplifies rounding differences)."""
+    pr = synth.make_problem(0)
+    g, o = make_pair(dm, pr)
+    c = pr.cfg
+    o32 = oracle.OracleDM(c.N, c.K, c.L, c.obj_h, c.obj_w, pr.positions, real="f32")
+    o32.set_data(pr.intensities, pr.probe0, pr.object0)
+    g.iterate(50); o.iterate(50); o32.iterate(50)
+    eg, eo, e32 = g.errors(), o.errors(), o32.errors()
+    curve = synth.rel_l2(eg[:, 0], eo[:, 0])
+    assert curve <= 1e-3, f"eps_F curve rel L2 {curve:.3e}"
+    for name, a, b, y in (("P", g.probe().cpu().numpy(), o.probe(), o32.probe()),
+                          ("O", g.object().cpu().numpy(), o.object(), o32.object())):
+        r, yard = synth.rel_l2(a, b), synth.rel_l2(y, b)
+        print(f"free run 50 it, {name}: GPU vs FP64 {r:.3e}; oracle FP32 vs FP64 {yard:.3e}")
+        assert r <= max(1e-3, 2 * yard), f"{name}: {r:.3e} vs yardstick {yard:.3e}"
+    g.close(); o.close(); o32.close()
+
+
+def test_run_to_run_determinism(dm):
+    pr = synth.make_problem(synth.CONFIGS[1].scaled(6, 5))
+    outs = []
+    for _ in range(2):
+        g, o = make_pair(dm, pr)
+        g.iterate(5)
+        outs.append((g.psi().cpu().numpy(), g.probe().cpu().numpy(), g.object().cpu().numpy(), g.errors()))
+        g.close(); o.close()
+    for a, b in zip(*outs):
+        assert np.array_equal(a, b)
+
+
+def test_fixed_point_noise_free(dm):
+    """Noise-free data, psi = P*O with the true P, O: one DM step leaves everything (nearly)
+    unchanged and every error ~ 0 (FP32 rounding level)."""
+    import dataclasses
+    cfg = dataclasses.replace(synth.CONFIGS[1].scaled(4, 4), photons=None)
+    pr = synth.make_problem(cfg)
+    pr.probe0[...] = pr.probe_true
+    pr.object0[...] = pr.object_true
+    g, o = make_pair(dm, pr)
+    g.iterate(1)
+    assert synth.rel_l2(g.probe().cpu().numpy(), pr.probe_true) < 1e-5
+    e = g.errors()[0]
+    assert e[0] < 1e-4 and e[1] < 1e-4
+    g.close(); o.close()
+
+
+def test_solve_host_matches_device_path(dm):
+    import torch
+    pr = synth.make_problem(synth.CONFIGS[1].scaled(4, 4))
+    c = pr.cfg
+    g, o = make_pair(dm, pr)
+    g.iterate(3)
+    P1, O1 = g.probe().cpu().numpy(), g.object().cpu().numpy()
+    h = dm.DMPlan(c.N, c.n_views, c.K, c.L, c.obj_h, c.obj_w, pr.positions).alloc_workspace()
+    Pout = np.empty_like(pr.probe0)
+    Oout = np.empty_like(pr.object0)
+    h.solve_host(pr.intensities, pr.probe0, pr.object0, 3, Pout, Oout)
+    assert np.array_equal(Pout, P1) and np.array_equal(Oout, O1)
+    g.close(); o.close(); h.close()
+    torch.cuda.synchronize()
