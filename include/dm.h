@@ -56,8 +56,9 @@ typedef enum {
     DM_PARAM_ALPHA_PROBE = 2, /* relative inertial factor a_P >= 0 of eq. (5); default 1e-3  */
     DM_PARAM_EPS_F = 3,       /* zero guard in eq. (4): scale = amp/sqrt(S+eps); default 1e-30 */
     DM_PARAM_PATH = 4         /* 0 = auto (default), 1 = force the staged (L2-scratch) path,
-                                 2 = force the fused per-frame path (DM_ERR_UNSUPPORTED at
-                                 dm_set_data if N > 128)                                     */
+                                 2 = force the fused shared-memory path (DM_ERR_UNSUPPORTED at
+                                 dm_set_data if N > 128), 3 = force the register-resident
+                                 path (DM_ERR_UNSUPPORTED at dm_set_data unless N = 128)     */
 } dm_param;
 
 /* Build the plan (HOST only, no CUDA call): validates, copies `positions` (HOST,
@@ -129,7 +130,8 @@ dm_status dm_solve_host(dm_plan *plan, const float *intensities_host, const floa
                         const float *object0_host, int n_iter, float *out_probe_host,
                         float *out_object_host, void *stream);
 
-/* Which path dm_iterate runs for this plan: 1 staged, 2 fused (valid after dm_set_data);
+/* Which path dm_iterate runs for this plan: 1 staged, 2 fused, 3 register-resident (valid
+ * after dm_set_data);
  * and how many kernels one iteration launches (the bench's gpu_launches claim).           */
 dm_status dm_plan_info(const dm_plan *plan, int *path, int *launches_per_iter);
 
@@ -146,6 +148,11 @@ dm_status dm_get_phase_ms(dm_plan *plan, float *out_ms4, int *iters);
  * swizzled tile addressing, digit-reversal map) single-threaded on the host for one
  * N x N frame and returns the spectrum in natural order.  in/out HOST c64 [N][N].       */
 dm_status dm_host_fft2(int N, const float *in_host, float *out_host, int inverse);
+/* Same hook for a named psi-update path: 1/2 = the shared-memory tile passes above, 3 = the
+ * register-resident 128 x 128 transform (csrc/dm_regfft.cuh: register passes, both exchange
+ * layouts, spectrum-layout table) emulated thread by thread, phase by phase.  N = 128 only
+ * for path 3 (UNSUPPORTED otherwise).                                                    */
+dm_status dm_host_fft2_path(int N, int path, const float *in_host, float *out_host, int inverse);
 
 const char *dm_status_string(dm_status s);
 const char *dm_last_error(const dm_plan *plan); /* plan may be NULL: last create error */

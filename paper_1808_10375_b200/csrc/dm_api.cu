@@ -18,6 +18,7 @@ constexpr int ERR_ROWS_CAP = 16384;
 constexpr size_t SCRATCH_TARGET = 48u << 20;     // staged path: spectra of one chunk stay in L2
 constexpr int COLS_SW = 8;                        // staged path: spectrum columns per CTA
 constexpr int PROF_MAX_ITERS = 4096;
+constexpr int REG_MAX_CTAS = 160;                 // path 3: upper bound on resident CTAs (B200: 148 SMs)
 
 thread_local std::string g_create_error;
 
@@ -30,10 +31,12 @@ struct dm_plan {
     std::vector<int32_t> pos;            // (y0,x0)
     std::vector<int32_t> tile_ptr, tile_views;
     int nty, ntx;
-    std::vector<int32_t> rev;            // digit reversal of the FFT passes
+    std::vector<int32_t> rev;            // digit reversal of the FFT passes (paths 1, 2)
+    std::vector<int32_t> spec;           // spectrum layout of the chosen path: storage position -> ky*N + kx
     std::vector<float> tw;               // N complex twiddles
     double beta, a_obj, a_probe, eps_f;
-    int path_req, path;                  // requested / chosen (1 staged, 2 fused)
+    int path_req, path;                  // requested / chosen (1 staged, 2 fused, 3 register-resident)
+    int reg_grid;                        // path 3: number of persistent CTAs (multiple of M)
     // probe reduction geometry
     int prb_blocks, prb_chunks, prb_chunk_len, fin_blocks;
     // staged geometry
@@ -44,7 +47,9 @@ struct dm_plan {
     float2 *psi, *Pbuf[2], *Obuf[2], *pnum, *scratch, *tw_d;
     float *amp, *pden, *den_tmp, *alphas, *partA, *partB, *partP, *partO;
     int2 *pos_d;
-    int *tile_ptr_d, *tile_views_d, *rev_d;
+    int *tile_ptr_d, *tile_views_d, *spec_d;
+    float2 *wy_d, *wx_d;                 // path 3 twiddle tables
+    float4 *sbuf;                        // path 3 mode-sum exchange (L2 resident)
     double *errors;
     float *stage_I;
     float2 *stage_P, *stage_O;
@@ -158,7 +163,8 @@ size_t carve(dm_plan *p, unsigned char *base)
     p->pden = (float *)take((size_t)p->prb_chunks * NN * sizeof(float));
     p->den_tmp = (float *)take((HW > NN ? HW : NN) * sizeof(float));
     p->alphas = (float *)take(2 * sizeof(float));
-    const size_t nA = (size_t)p->nA * 2 > MV * 4 ? (size_t)p->nA * 2 : MV * 4;
+    size_t nA = (size_t)p->nA * 2 > MV * 4 ? (size_t)p->nA * 2 : MV * 4;
+    if (nA < (size_t)REG_MAX_CTAS * 4) nA = (size_t)REG_MAX_CTAS * 4;
     p->partA = (float *)take(nA * sizeof(float));
     p->partB = (float *)take((size_t)p->nB * 2 * sizeof(float));
     p->partP = (float *)take((size_t)p->fin_blocks * p->K * 2 * sizeof(float));
@@ -166,7 +172,10 @@ size_t carve(dm_plan *p, unsigned char *base)
     p->pos_d = (int2 *)take((size_t)p->n_views * sizeof(int2));
     p->tile_ptr_d = (int *)take(p->tile_ptr.size() * sizeof(int));
     p->tile_views_d = (int *)take((p->tile_views.size() + 1) * sizeof(int));
-    p->rev_d = (int *)take(p->N * sizeof(int));
+    p->spec_d = (int *)take(NN * sizeof(int));
+    p->wy_d = (float2 *)take(128 * sizeof(float2));
+    p->wx_d = (float2 *)take(128 * sizeof(float2));
+    p->sbuf = (float4 *)take(p->N == 128 ? (size_t)2 * REG_MAX_CTAS * 8 * dmreg::RNT * sizeof(float4) : 0);
     p->tw_d = (float2 *)take(p->N * sizeof(float2));
     p->errors = (double *)take((size_t)ERR_ROWS_CAP * (2 + p->K + p->L) * sizeof(double));
     p->scratch = (float2 *)take((size_t)p->chunk_views * p->M * NN * sizeof(float2));
@@ -237,8 +246,71 @@ template <int N> dm_status launch_staged(dm_plan *plan, cudaStream_t st)
     return DM_OK;
 }
 
+// path 3: persistent register-resident kernel, cluster = the M mode frames of a view
+template <int MT> dm_status launch_regfft_t(dm_plan *plan, cudaStream_t st, bool query_only)
+{
+    auto kern = dmreg::regfft128_kernel<MT>;
+    static bool attr_done = false;
+    if (!attr_done) {
+        CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, dmreg::REG_SMEM_V1));
+        attr_done = true;
+    }
+    cudaLaunchConfig_t cfg;
+    memset(&cfg, 0, sizeof cfg);
+    cfg.blockDim = dim3(dmreg::RNT);
+    cfg.dynamicSmemBytes = dmreg::REG_SMEM_V1;
+    cfg.stream = st;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeClusterDimension;
+    at[0].val.clusterDim.x = (unsigned)plan->M;
+    at[0].val.clusterDim.y = 1;
+    at[0].val.clusterDim.z = 1;
+    cfg.attrs = at;
+    cfg.numAttrs = plan->M > 1 ? 1 : 0;
+    if (query_only) {
+        int ncl = 0;
+        if (plan->M > 1) {
+            cfg.gridDim = dim3((unsigned)plan->M);
+            CU(cudaOccupancyMaxActiveClusters(&ncl, kern, &cfg));
+        } else {
+            int dev = 0, sms = 0, per = 0;
+            CU(cudaGetDevice(&dev));
+            CU(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+            CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per, kern, dmreg::RNT, dmreg::REG_SMEM_V1));
+            ncl = sms * per;
+        }
+        if (ncl < 1) return fail(plan, DM_ERR_CUDA, "register-resident kernel: no cluster of %d CTAs fits", plan->M);
+        if (ncl > plan->n_views) ncl = plan->n_views;
+        if (ncl * plan->M > REG_MAX_CTAS) ncl = REG_MAX_CTAS / plan->M;
+        plan->reg_grid = ncl * plan->M;
+        return DM_OK;
+    }
+    dmreg::RegArgs a;
+    memset(&a, 0, sizeof a);
+    a.n_views = plan->n_views; a.K = plan->K; a.L = plan->L; a.H = plan->H; a.W = plan->W;
+    a.pos = plan->pos_d; a.P = plan->Pbuf[plan->curP]; a.O = plan->Obuf[plan->curO];
+    a.psi = plan->psi; a.amp = plan->amp; a.wy = plan->wy_d; a.wx = plan->wx_d;
+    a.sbuf = plan->sbuf; a.part = plan->partA;
+    a.beta = (float)plan->beta; a.eps = (float)plan->eps_f;
+    cfg.gridDim = dim3((unsigned)plan->reg_grid);
+    CU(cudaLaunchKernelEx(&cfg, kern, a));
+    return DM_OK;
+}
+
+dm_status launch_regfft(dm_plan *plan, cudaStream_t st, bool query_only)
+{
+    switch (plan->M) {
+    case 1: return launch_regfft_t<1>(plan, st, query_only);
+    case 2: return launch_regfft_t<2>(plan, st, query_only);
+    case 3: return launch_regfft_t<3>(plan, st, query_only);
+    case 4: return launch_regfft_t<4>(plan, st, query_only);
+    default: return launch_regfft_t<0>(plan, st, query_only);
+    }
+}
+
 dm_status launch_psi_update(dm_plan *plan, cudaStream_t st)
 {
+    if (plan->path == 3) return launch_regfft(plan, st, false);
     if (plan->path == 2) {
         if (plan->N == 64) return launch_fused<64, 256>(plan, st);
         return launch_fused<128, 512>(plan, st);
@@ -355,7 +427,7 @@ dm_status dm_plan_set_param(dm_plan *plan, dm_param which, double v)
     case DM_PARAM_ALPHA_OBJ: if (v < 0) break; plan->a_obj = v; return DM_OK;
     case DM_PARAM_ALPHA_PROBE: if (v < 0) break; plan->a_probe = v; return DM_OK;
     case DM_PARAM_EPS_F: if (v < 0) break; plan->eps_f = v; return DM_OK;
-    case DM_PARAM_PATH: if (v != 0 && v != 1 && v != 2) break; plan->path_req = (int)v; return DM_OK;
+    case DM_PARAM_PATH: if (v != 0 && v != 1 && v != 2 && v != 3) break; plan->path_req = (int)v; return DM_OK;
     default: return fail(plan, DM_ERR_INVALID_ARG, "unknown parameter %d", (int)which);
     }
     return fail(plan, DM_ERR_INVALID_ARG, "parameter %d: value %g out of range", (int)which, v);
@@ -388,24 +460,53 @@ dm_status dm_set_data(dm_plan *plan, const float *intensities, const float *prob
     if (s != DM_OK) return s;
     if (!intensities || !probe0 || !object0) return fail(plan, DM_ERR_INVALID_ARG, "NULL data pointer");
     int path = plan->path_req;
-    if (path == 0) path = (plan->N <= 128) ? 2 : 1;
+    if (path == 0) path = plan->N == 128 ? 3 : (plan->N < 128 ? 2 : 1);
     if (path == 2 && plan->N > 128)
         return fail(plan, DM_ERR_UNSUPPORTED, "fused per-frame path needs N <= 128 (N = %d)", plan->N);
+    if (path == 3 && plan->N != 128)
+        return fail(plan, DM_ERR_UNSUPPORTED, "register-resident path needs N = 128 (N = %d)", plan->N);
     plan->path = path;
     cudaStream_t st = (cudaStream_t)stream;
     const size_t NN = (size_t)plan->N * plan->N, HW = (size_t)plan->H * plan->W;
+    // spectrum layout of the chosen path (where sqrt(I) has to sit)
+    plan->spec.assign(NN, 0);
+    if (path == 3) {
+        for (int tid = 0; tid < dmreg::RNT; ++tid)
+            for (int e = 0; e < dmreg::REPT; ++e) plan->spec[dmreg::spec_pos(tid, e)] = dmreg::spec_freq(tid, e);
+        std::vector<float> wy(256), wx(256);
+        for (int w = 0; w < 16; ++w)
+            for (int q = 0; q < 8; ++q) {
+                const double ang = -2.0 * M_PI * (double)(w * q) / 128.0;
+                wy[2 * (w * 8 + q)] = (float)std::cos(ang);
+                wy[2 * (w * 8 + q) + 1] = (float)std::sin(ang);
+            }
+        for (int t = 0; t < 32; ++t)
+            for (int r = 0; r < 4; ++r) {
+                const double ang = -2.0 * M_PI * (double)(t * r) / 128.0;
+                wx[2 * (t * 4 + r)] = (float)std::cos(ang);
+                wx[2 * (t * 4 + r) + 1] = (float)std::sin(ang);
+            }
+        CU(cudaMemcpyAsync(plan->wy_d, wy.data(), 256 * sizeof(float), cudaMemcpyHostToDevice, st));
+        CU(cudaMemcpyAsync(plan->wx_d, wx.data(), 256 * sizeof(float), cudaMemcpyHostToDevice, st));
+        CU(cudaStreamSynchronize(st));          // wy / wx are stack-owned host buffers
+        dm_status qs = launch_regfft(plan, st, true);
+        if (qs != DM_OK) return qs;
+    } else {
+        for (int py = 0; py < plan->N; ++py)
+            for (int px = 0; px < plan->N; ++px) plan->spec[(size_t)py * plan->N + px] = plan->rev[py] * plan->N + plan->rev[px];
+    }
     CU(cudaMemcpyAsync(plan->pos_d, plan->pos.data(), plan->pos.size() * sizeof(int32_t), cudaMemcpyHostToDevice, st));
     CU(cudaMemcpyAsync(plan->tile_ptr_d, plan->tile_ptr.data(), plan->tile_ptr.size() * sizeof(int32_t), cudaMemcpyHostToDevice, st));
     if (!plan->tile_views.empty())
         CU(cudaMemcpyAsync(plan->tile_views_d, plan->tile_views.data(), plan->tile_views.size() * sizeof(int32_t), cudaMemcpyHostToDevice, st));
-    CU(cudaMemcpyAsync(plan->rev_d, plan->rev.data(), plan->rev.size() * sizeof(int32_t), cudaMemcpyHostToDevice, st));
+    CU(cudaMemcpyAsync(plan->spec_d, plan->spec.data(), plan->spec.size() * sizeof(int32_t), cudaMemcpyHostToDevice, st));
     CU(cudaMemcpyAsync(plan->tw_d, plan->tw.data(), plan->tw.size() * sizeof(float), cudaMemcpyHostToDevice, st));
     plan->curP = plan->curO = 0;
     CU(cudaMemcpyAsync(plan->Pbuf[0], probe0, plan->K * NN * sizeof(float2), cudaMemcpyDeviceToDevice, st));
     CU(cudaMemcpyAsync(plan->Obuf[0], object0, plan->L * HW * sizeof(float2), cudaMemcpyDeviceToDevice, st));
     CU(cudaMemsetAsync(plan->alphas, 0, 2 * sizeof(float), st));
     const size_t total = (size_t)plan->n_views * NN;
-    amp_permute_kernel<<<148 * 8, 256, 0, st>>>(plan->N, intensities, plan->rev_d, plan->amp, total);
+    amp_permute_kernel<<<148 * 8, 256, 0, st>>>(plan->N, intensities, plan->spec_d, plan->amp, total);
     psi_init_kernel<<<dim3((unsigned)((NN + 1023) / 1024), (unsigned)(plan->n_views * plan->M)), 256, 0, st>>>(
         plan->N, plan->K, plan->L, plan->H, plan->W, plan->pos_d, plan->Pbuf[0], plan->Obuf[0], plan->psi);
     CU(cudaGetLastError());
@@ -454,7 +555,10 @@ dm_status dm_iterate(dm_plan *plan, int n_iter, void *stream)
         if (s != DM_OK) return s;
         if (ev) CU(cudaEventRecord(ev[3], st));
         ErrArgs e;                                                                   // S9
-        if (plan->path == 2) {
+        if (plan->path == 3) {
+            e.pF = plan->partA;     e.nF = plan->reg_grid; e.sF = 4;
+            e.pS = plan->partA + 2; e.nS = plan->reg_grid; e.sS = 4;
+        } else if (plan->path == 2) {
             e.pF = plan->partA;     e.nF = plan->n_views * plan->M; e.sF = 4;
             e.pS = plan->partA + 2; e.nS = plan->n_views * plan->M; e.sS = 4;
         } else {
@@ -619,11 +723,11 @@ dm_status dm_get_phase_ms(dm_plan *plan, float *out_ms4, int *iters)
 dm_status dm_plan_info(const dm_plan *plan, int *path, int *launches_per_iter)
 {
     if (!plan) return DM_ERR_INVALID_ARG;
-    int p = plan->path ? plan->path : (plan->path_req ? plan->path_req : (plan->N <= 128 ? 2 : 1));
+    int p = plan->path ? plan->path : (plan->path_req ? plan->path_req : (plan->N == 128 ? 3 : (plan->N < 128 ? 2 : 1)));
     if (path) *path = p;
     if (launches_per_iter) {
         const int chunks = (plan->n_views + plan->chunk_views - 1) / plan->chunk_views;
-        *launches_per_iter = (p == 2 ? 1 : 3 * chunks) + 4;
+        *launches_per_iter = (p >= 2 ? 1 : 3 * chunks) + 4;
     }
     return DM_OK;
 }
@@ -663,9 +767,77 @@ template <int N> void host_fft2(const float *in, float *out, int inverse)
         for (int e = 0; e < N * N; ++e) dst[e] = make_float2(tile[swz(e)].x * s, tile[swz(e)].y * s);
     }
 }
+// path 3 (dm_regfft.cuh): 512 emulated threads, phase by phase (a phase boundary = a barrier)
+void host_fft2_reg(const float *in, float *out, int inverse)
+{
+    using namespace dmreg;
+    std::vector<float2> regs((size_t)RNT * REPT);
+    std::vector<float4> xbuf_v(XBUF_BYTES / 16);
+    unsigned char *xbuf = reinterpret_cast<unsigned char *>(xbuf_v.data());
+    std::vector<float2> wy(128), wx(128);
+    for (int w = 0; w < 16; ++w)
+        for (int q = 0; q < 8; ++q) {
+            const double ang = -2.0 * M_PI * (double)(w * q) / 128.0;
+            wy[w * 8 + q] = make_float2((float)std::cos(ang), (float)std::sin(ang));
+        }
+    for (int t = 0; t < 32; ++t)
+        for (int r = 0; r < 4; ++r) {
+            const double ang = -2.0 * M_PI * (double)(t * r) / 128.0;
+            wx[t * 4 + r] = make_float2((float)std::cos(ang), (float)std::sin(ang));
+        }
+    auto U = [&](int tid) -> float2(&)[32] { return *reinterpret_cast<float2(*)[32]>(&regs[(size_t)tid * REPT]); };
+    const float2 *src = reinterpret_cast<const float2 *>(in);
+    float2 *dst = reinterpret_cast<float2 *>(out);
+    auto exch1 = [&]() {
+        for (int rho = 0; rho < 2; ++rho) {
+            for (int tid = 0; tid < RNT; ++tid) x1_write(U(tid), rho, tid & 31, xbuf + (tid >> 5) * X1_WARP);
+            for (int tid = 0; tid < RNT; ++tid) x1_read(U(tid), rho, tid & 31, xbuf + (tid >> 5) * X1_WARP);
+        }
+    };
+    auto exch2 = [&]() {
+        for (int z = 0; z < 2; ++z) {
+            for (int tid = 0; tid < RNT; ++tid) x2_write(U(tid), z, tid >> 5, tid & 31, reinterpret_cast<float2 *>(xbuf));
+            for (int tid = 0; tid < RNT; ++tid) x2_read(U(tid), z, tid >> 5, tid & 31, reinterpret_cast<const float2 *>(xbuf));
+        }
+    };
+    if (!inverse) {
+        for (int tid = 0; tid < RNT; ++tid)
+            for (int a = 0; a < REPT; ++a) U(tid)[a] = src[l0_pixel(tid, a)];
+        for (int tid = 0; tid < RNT; ++tid) pass1_fwd(U(tid), &wy[(tid >> 5) * 8], &wx[(tid & 31) * 4]);
+        exch1();
+        for (int tid = 0; tid < RNT; ++tid) pass2<false>(U(tid));
+        exch2();
+        for (int tid = 0; tid < RNT; ++tid) pass3<false>(U(tid));
+        for (int tid = 0; tid < RNT; ++tid)
+            for (int e = 0; e < REPT; ++e) dst[spec_freq(tid, e)] = U(tid)[e];
+    } else {
+        for (int tid = 0; tid < RNT; ++tid)
+            for (int e = 0; e < REPT; ++e) U(tid)[e] = src[spec_freq(tid, e)];
+        for (int tid = 0; tid < RNT; ++tid) pass3<true>(U(tid));
+        exch2();
+        for (int tid = 0; tid < RNT; ++tid) pass2<true>(U(tid));
+        exch1();
+        for (int tid = 0; tid < RNT; ++tid) pass1_inv(U(tid), &wy[(tid >> 5) * 8], &wx[(tid & 31) * 4]);
+        const float s = 1.f / (float)RNN;
+        for (int tid = 0; tid < RNT; ++tid)
+            for (int a = 0; a < REPT; ++a) dst[l0_pixel(tid, a)] = make_float2(U(tid)[a].x * s, U(tid)[a].y * s);
+    }
+}
 } // namespace
 
 extern "C" {
+
+dm_status dm_host_fft2_path(int N, int path, const float *in_host, float *out_host, int inverse)
+{
+    if (!in_host || !out_host) return DM_ERR_INVALID_ARG;
+    if (path == 3) {
+        if (N != 128) return DM_ERR_UNSUPPORTED;
+        host_fft2_reg(in_host, out_host, inverse);
+        return DM_OK;
+    }
+    if (path != 1 && path != 2) return DM_ERR_INVALID_ARG;
+    return dm_host_fft2(N, in_host, out_host, inverse);
+}
 
 dm_status dm_host_fft2(int N, const float *in_host, float *out_host, int inverse)
 {

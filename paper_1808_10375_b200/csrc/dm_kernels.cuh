@@ -16,6 +16,7 @@
 #include <stdint.h>
 
 #include "dm_fft.cuh"
+#include "dm_regfft.cuh"
 
 namespace cg = cooperative_groups;
 using namespace dmfft;
@@ -61,15 +62,15 @@ __device__ __forceinline__ float4 po2(float4 p, float2 o0, float2 o1)
 }
 
 // ------------------------------------------------------------- set_data kernels -----
-// amp[v][py][px] = sqrt(I[v][rev[py]][rev[px]])  (spectrum layout of the kernels)
-__global__ void amp_permute_kernel(int N, const float *__restrict__ inten, const int *__restrict__ rev,
+// amp[v][p] = sqrt(I[v][spec[p]]): sqrt(I) stored once in the spectrum layout of the chosen
+// psi-update path (spec[p] = natural-order frequency index ky*N + kx held at storage position p)
+__global__ void amp_permute_kernel(int N, const float *__restrict__ inten, const int *__restrict__ spec,
                                    float *__restrict__ amp, size_t total)
 {
     const size_t NN = (size_t)N * N;
     for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < total; i += (size_t)gridDim.x * blockDim.x) {
         const size_t v = i / NN;
-        const int p = (int)(i % NN), py = p / N, px = p % N;
-        amp[i] = sqrtf(inten[v * NN + (size_t)rev[py] * N + rev[px]]);
+        amp[i] = sqrtf(inten[v * NN + spec[i % NN]]);
     }
 }
 

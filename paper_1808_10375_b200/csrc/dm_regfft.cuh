@@ -1,0 +1,427 @@
+// dm_regfft.cuh -- register-resident 128 x 128 frame transform of the psi update (steps S1-S6
+// of DESIGN.md; eqs. (2)-(4) of arXiv:1808.10375).  Included by dm_kernels.cuh.
+//
+// One CTA of 512 threads holds ONE whole 128 x 128 complex64 mode frame in registers (32
+// elements per thread).  The 2-D FFT is three register passes with two shared-memory exchanges:
+//
+//   L0 (load/store layout, coalesced rows):  thread (warp w, lane t), register a = 4 i + r
+//        holds pixel  y = w + 16 i (i < 8),  x = t + 32 r (r < 4)
+//   pass 1   radix-8 along y over i  (-> q),   twiddle w128^(w q)
+//            radix-4 along x over r  (-> r'),  twiddle w128^(t r')          register a' = 4 q + r'
+//   exch. 1  32 x 32 transpose inside each warp: (lane t, reg a') -> (lane a', reg t)
+//   pass 2   radix-32 along x over t (-> c):   kx = r' + 4 c               x is finished
+//   exch. 2  16 x 16 transpose across the warps, lane fixed, the register bit z = c >> 4 stays:
+//            (warp w, reg 16 z + c') -> (warp c', reg 16 z + w)
+//   pass 3   radix-16 along y over w (-> k2):  ky = q + 8 k2               y is finished
+//
+//   spectrum layout: thread (warp w', lane t' = 4 q + r'), register e = 16 z + k2 holds
+//        F[ky = q + 8 k2][kx = r' + 4 (w' + 16 z)]
+//
+// The inverse runs the mirrored passes (both exchanges are involutions), ending in L0.  The
+// Fourier-modulus step (eq. (4)) is pointwise, so it runs in the spectrum layout; sqrt(I) is
+// stored once in that layout (spec_index table, dm_set_data).
+//
+// Every function here is __host__ __device__: tests run exactly this code on the CPU through
+// dm_host_fft2 (512 emulated threads, phase by phase) before anything goes to a GPU.
+#pragma once
+#include <cuda_runtime.h>
+
+#include "dm_fft.cuh"
+
+namespace dmreg {
+
+using namespace dmfft;
+
+constexpr int RN = 128, RNN = RN * RN, RNT = 512, REPT = 32;
+// exchange buffer: 16 warps x (2 blocks of 16 rows x 144 B) for exchange 1, 64 KiB for exchange 2
+constexpr int X1_ROW = 144, X1_BLK = 16 * X1_ROW, X1_WARP = 2 * X1_BLK;       // bytes
+constexpr int XBUF_BYTES = 16 * X1_WARP;                                       // 73728 >= 65536
+
+// cos / sin of 2 pi m / 32
+__device__ __host__ constexpr float c32(int m)
+{
+    constexpr float C[32] = {1.f, 0.98078528040323043f, 0.92387953251128674f, 0.83146961230254524f, 0.70710678118654757f,
+        0.55557023301960229f, 0.38268343236508984f, 0.19509032201612833f, 0.f, -0.19509032201612819f, -0.38268343236508973f,
+        -0.55557023301960196f, -0.70710678118654746f, -0.83146961230254535f, -0.92387953251128674f, -0.98078528040323043f,
+        -1.f, -0.98078528040323043f, -0.92387953251128685f, -0.83146961230254546f, -0.70710678118654768f,
+        -0.55557023301960218f, -0.38268343236509034f, -0.19509032201612866f, 0.f, 0.1950903220161283f, 0.38268343236509f,
+        0.55557023301960184f, 0.70710678118654735f, 0.83146961230254524f, 0.92387953251128652f, 0.98078528040323032f};
+    return C[m & 31];
+}
+__device__ __host__ constexpr float s32(int m) { return c32(m - 8); }
+
+// a * w32^M (forward: exp(-2 pi i M/32); inverse: conjugate), M a compile-time constant
+template <bool INV, int M> DM_HD float2 mul_w32(float2 a)
+{
+    constexpr int m = M & 31;
+    if (m == 0) return a;
+    if (m == 16) return make_float2(-a.x, -a.y);
+    if (m == 8) return mul_mi<INV>(a);
+    if (m == 24) return mul_mi<!INV>(a);
+    constexpr float c = c32(m), s = s32(m);
+    return INV ? make_float2(a.x * c - a.y * s, a.x * s + a.y * c)
+               : make_float2(a.x * c + a.y * s, a.y * c - a.x * s);
+}
+
+// natural-order 32-point DFT in registers: n = 8 n1 + n2, k = k1 + 4 k2
+template <bool INV> DM_HD void dft32(float2 (&x)[32])
+{
+#pragma unroll
+    for (int n2 = 0; n2 < 8; ++n2) dft4<INV>(x[n2], x[8 + n2], x[16 + n2], x[24 + n2]);   // -> x[8 k1 + n2]
+#define DM_TW(K1, N2) x[8 * K1 + N2] = mul_w32<INV, K1 * N2>(x[8 * K1 + N2]);
+#define DM_TWROW(K1) DM_TW(K1, 1) DM_TW(K1, 2) DM_TW(K1, 3) DM_TW(K1, 4) DM_TW(K1, 5) DM_TW(K1, 6) DM_TW(K1, 7)
+    DM_TWROW(1) DM_TWROW(2) DM_TWROW(3)
+#undef DM_TWROW
+#undef DM_TW
+    float2 y[32];
+#pragma unroll
+    for (int k1 = 0; k1 < 4; ++k1) {
+        float2 v[8];
+#pragma unroll
+        for (int n2 = 0; n2 < 8; ++n2) v[n2] = x[8 * k1 + n2];
+        dft8<INV>(v);
+#pragma unroll
+        for (int k2 = 0; k2 < 8; ++k2) y[k1 + 4 * k2] = v[k2];
+    }
+#pragma unroll
+    for (int k = 0; k < 32; ++k) x[k] = y[k];
+}
+
+// ---- register passes ------------------------------------------------------------------
+// wy[q] = w128^(w q) (q < 8, per warp), wx[r'] = w128^(t r') (r' < 4, per lane); forward sign.
+DM_HD void pass1_fwd(float2 (&u)[32], const float2 *wy, const float2 *wx)
+{
+#pragma unroll
+    for (int r = 0; r < 4; ++r) {
+        float2 v[8];
+#pragma unroll
+        for (int i = 0; i < 8; ++i) v[i] = u[4 * i + r];
+        dft8<false>(v);
+        u[r] = v[0];
+#pragma unroll
+        for (int q = 1; q < 8; ++q) u[4 * q + r] = cmul(v[q], wy[q]);
+    }
+#pragma unroll
+    for (int q = 0; q < 8; ++q) {
+        dft4<false>(u[4 * q], u[4 * q + 1], u[4 * q + 2], u[4 * q + 3]);
+#pragma unroll
+        for (int rp = 1; rp < 4; ++rp) u[4 * q + rp] = cmul(u[4 * q + rp], wx[rp]);
+    }
+}
+
+DM_HD void pass1_inv(float2 (&u)[32], const float2 *wy, const float2 *wx)
+{
+#pragma unroll
+    for (int q = 0; q < 8; ++q) {
+#pragma unroll
+        for (int rp = 1; rp < 4; ++rp) u[4 * q + rp] = cmulc(u[4 * q + rp], wx[rp]);
+        dft4<true>(u[4 * q], u[4 * q + 1], u[4 * q + 2], u[4 * q + 3]);
+    }
+#pragma unroll
+    for (int r = 0; r < 4; ++r) {
+        float2 v[8];
+        v[0] = u[r];
+#pragma unroll
+        for (int q = 1; q < 8; ++q) v[q] = cmulc(u[4 * q + r], wy[q]);
+        dft8<true>(v);
+#pragma unroll
+        for (int i = 0; i < 8; ++i) u[4 * i + r] = v[i];
+    }
+}
+
+template <bool INV> DM_HD void pass2(float2 (&u)[32]) { dft32<INV>(u); }
+
+template <bool INV> DM_HD void pass3(float2 (&u)[32])
+{
+#pragma unroll
+    for (int z = 0; z < 2; ++z) {
+        float2 v[16];
+#pragma unroll
+        for (int i = 0; i < 16; ++i) v[i] = u[16 * z + i];
+        dft16<INV>(v);
+#pragma unroll
+        for (int i = 0; i < 16; ++i) u[16 * z + i] = v[i];
+    }
+}
+
+// ---- exchange 1: 32 x 32 transpose inside a warp, two rounds of 16 registers ----------
+// Round rho moves the elements (reg a', lane b) with (a' >> 4) == (b >> 4) ^ rho, so every lane
+// writes 16 registers and reads 16 registers per round (4.5 KiB of buffer per warp).  Rows of
+// 16 elements are padded to 144 B: 64-bit stores of a row and 128-bit loads down a column
+// are both bank-conflict free.  wbuf = this warp's 4608-byte region.
+DM_HD void x1_write(const float2 (&u)[32], int rho, int t, unsigned char *wbuf)
+{
+    const int h = (t >> 4) ^ rho;                   // which register half this lane sends
+    unsigned char *p = wbuf + h * X1_BLK + (t & 15) * 8;
+    if (h == 0) {
+#pragma unroll
+        for (int j = 0; j < 16; ++j) *reinterpret_cast<float2 *>(p + j * X1_ROW) = u[j];
+    } else {
+#pragma unroll
+        for (int j = 0; j < 16; ++j) *reinterpret_cast<float2 *>(p + j * X1_ROW) = u[16 + j];
+    }
+}
+
+DM_HD void x1_read(float2 (&u)[32], int rho, int t, const unsigned char *wbuf)
+{
+    const int h = (t >> 4) ^ rho;                   // which register half this lane receives
+    const unsigned char *p = wbuf + (t >> 4) * X1_BLK + (t & 15) * X1_ROW;
+    if (h == 0) {
+#pragma unroll
+        for (int b = 0; b < 16; b += 2) {
+            const float4 v = *reinterpret_cast<const float4 *>(p + b * 8);
+            u[b] = make_float2(v.x, v.y);
+            u[b + 1] = make_float2(v.z, v.w);
+        }
+    } else {
+#pragma unroll
+        for (int b = 0; b < 16; b += 2) {
+            const float4 v = *reinterpret_cast<const float4 *>(p + b * 8);
+            u[16 + b] = make_float2(v.x, v.y);
+            u[16 + b + 1] = make_float2(v.z, v.w);
+        }
+    }
+}
+
+// ---- exchange 2: (warp w, reg 16 z + c') <-> (warp c', reg 16 z + w), lane fixed -------
+// One round per z through a 64 KiB buffer: element (c', w, lane) at ((c' 16 + w) 32 + lane) 8 B.
+DM_HD void x2_write(const float2 (&u)[32], int z, int w, int t, float2 *buf)
+{
+    float2 *p = buf + w * 32 + t;
+    if (z == 0) {
+#pragma unroll
+        for (int c = 0; c < 16; ++c) p[c * 512] = u[c];
+    } else {
+#pragma unroll
+        for (int c = 0; c < 16; ++c) p[c * 512] = u[16 + c];
+    }
+}
+
+DM_HD void x2_read(float2 (&u)[32], int z, int w, int t, const float2 *buf)
+{
+    const float2 *p = buf + w * 512 + t;
+    if (z == 0) {
+#pragma unroll
+        for (int i = 0; i < 16; ++i) u[i] = p[i * 32];
+    } else {
+#pragma unroll
+        for (int i = 0; i < 16; ++i) u[16 + i] = p[i * 32];
+    }
+}
+
+// storage position (float index inside a frame's N*N block) of register e of thread tid in the
+// spectrum layout, as written with one float4 per 4 registers: [e >> 2][tid][e & 3]
+DM_HD int spec_pos(int tid, int e) { return ((e >> 2) * RNT + tid) * 4 + (e & 3); }
+// natural-order linear frequency index ky * 128 + kx that (tid, e) holds after the forward passes
+DM_HD int spec_freq(int tid, int e)
+{
+    const int w = tid >> 5, t = tid & 31, q = t >> 2, rp = t & 3, z = e >> 4, k2 = e & 15;
+    return (q + 8 * k2) * RN + rp + 4 * (w + 16 * z);
+}
+// L0 pixel (linear index y * 128 + x) of register a of thread tid
+DM_HD int l0_pixel(int tid, int a)
+{
+    const int w = tid >> 5, t = tid & 31;
+    return (w + 16 * (a >> 2)) * RN + t + 32 * (a & 3);
+}
+
+} // namespace dmreg
+
+// =========================================================================================
+// The kernel (device only)
+// =========================================================================================
+#ifdef __CUDACC__
+#include <cooperative_groups.h>
+
+namespace dmreg {
+
+struct RegArgs {
+    int n_views, K, L, H, W;
+    const int2 *pos;            // (y0, x0) per view
+    const float2 *P;            // [K][128][128]   current probe
+    const float2 *O;            // [L][H][W]       current object
+    float2 *psi;                // [n_views][K][L][128][128], updated in place
+    const float *amp;           // [n_views][128*128] sqrt(I) in the spectrum layout (spec_pos)
+    const float2 *wy;           // [16][8]  w128^(w q)
+    const float2 *wx;           // [32][4]  w128^(t r')
+    float4 *sbuf;               // [2][grid][8][512]  |F|^2 of every resident CTA (mode-sum exchange, L2)
+    float *part;                // [grid][4]  (eF_num, eF_den, epsi_num, epsi_den) partial sums
+    float beta, eps;
+};
+
+constexpr int REG_SMEM_V1 = XBUF_BYTES + RNN * 8 + 2048;     // exchange + P*O + twiddles
+
+__device__ __forceinline__ float abs2_rn(float2 f) { return __fmaf_rn(f.y, f.y, __fmul_rn(f.x, f.x)); }
+
+// Persistent CTAs; cluster = the M = K*L mode frames of one view (cluster rank m = mode index),
+// cluster c processes views c, c + n_clusters, ...  MT = compile-time M (0: run-time M).
+template <int MT>
+__global__ void __launch_bounds__(RNT, 1) regfft128_kernel(const RegArgs a)
+{
+    namespace cg = cooperative_groups;
+    extern __shared__ __align__(16) unsigned char smem[];
+    unsigned char *xbuf = smem;
+    float2 *pobuf = reinterpret_cast<float2 *>(smem + XBUF_BYTES);
+    float2 *s_wy = reinterpret_cast<float2 *>(smem + XBUF_BYTES + RNN * 8);
+    float2 *s_wx = s_wy + 128;
+    __shared__ float red[4 * 32];
+
+    const int tid = threadIdx.x, w = tid >> 5, t = tid & 31;
+    const int M = MT ? MT : a.K * a.L;
+    const int m = blockIdx.x % M, cl = blockIdx.x / M, ncl = gridDim.x / M;
+    const int k = m / a.L, l = m % a.L;
+    if (tid < 128) s_wy[tid] = a.wy[tid];
+    else if (tid < 256) s_wx[tid - 128] = a.wx[tid - 128];
+    __syncthreads();
+
+    unsigned char *wbuf = xbuf + w * X1_WARP;
+    float2 *xb2 = reinterpret_cast<float2 *>(xbuf);
+    const float2 *Pk = a.P + (size_t)k * RNN + w * RN + t;
+    const float cfac = a.beta > 0.f ? 1.f / (float)RNN : 0.f;
+    float e0 = 0.f, e1 = 0.f, e2 = 0.f, e3 = 0.f;
+    int par = 0;
+
+    for (int view = cl; view < a.n_views; view += ncl, par ^= 1) {
+        const int2 p0 = a.pos[view];
+        float2 *psi_f = a.psi + ((size_t)view * M + m) * RNN + w * RN + t;
+        const float2 *Ow = a.O + (size_t)l * a.H * a.W + (size_t)(p0.x + w) * a.W + p0.y + t;
+        float2 u[32];
+        // ---- S1 + S2: R = 2 P O - psi in L0; P*O parked in shared memory ----
+#pragma unroll
+        for (int r = 0; r < 32; ++r) u[r] = psi_f[(r >> 2) * 16 * RN + (r & 3) * 32];
+#pragma unroll
+        for (int i = 0; i < 8; ++i) {
+            float2 p[4], o[4];
+#pragma unroll
+            for (int r = 0; r < 4; ++r) {
+                p[r] = __ldg(Pk + i * 16 * RN + r * 32);
+                o[r] = __ldg(Ow + (size_t)i * 16 * a.W + r * 32);
+            }
+#pragma unroll
+            for (int r = 0; r < 4; ++r) {
+                const float2 po = cmul(p[r], o[r]);
+                pobuf[(4 * i + r) * RNT + tid] = po;
+                u[4 * i + r] = make_float2(2.f * po.x - u[4 * i + r].x, 2.f * po.y - u[4 * i + r].y);
+            }
+        }
+        // ---- S3: forward 2-D FFT ----
+        {
+            float2 wy[8], wx[4];
+#pragma unroll
+            for (int q = 0; q < 8; ++q) wy[q] = s_wy[w * 8 + q];
+#pragma unroll
+            for (int r = 0; r < 4; ++r) wx[r] = s_wx[t * 4 + r];
+            pass1_fwd(u, wy, wx);
+        }
+#pragma unroll
+        for (int rho = 0; rho < 2; ++rho) {
+            x1_write(u, rho, t, wbuf);
+            __syncwarp();
+            x1_read(u, rho, t, wbuf);
+            __syncwarp();
+        }
+        pass2<false>(u);
+#pragma unroll
+        for (int z = 0; z < 2; ++z) {
+            __syncthreads();
+            x2_write(u, z, w, t, xb2);
+            __syncthreads();
+            x2_read(u, z, w, t, xb2);
+        }
+        pass3<false>(u);
+        // ---- S4: mode-summed modulus constraint (|F|^2 exchanged through L2) ----
+        {
+            float4 *mine = a.sbuf + (((size_t)par * gridDim.x + blockIdx.x) * 8) * RNT + tid;
+            if (M > 1) {
+#pragma unroll
+                for (int j = 0; j < 8; ++j)
+                    mine[j * RNT] = make_float4(abs2_rn(u[4 * j]), abs2_rn(u[4 * j + 1]), abs2_rn(u[4 * j + 2]), abs2_rn(u[4 * j + 3]));
+                cg::this_cluster().sync();
+            } else {
+                __syncthreads();
+            }
+            const float4 *ampv = reinterpret_cast<const float4 *>(a.amp + (size_t)view * RNN) + tid;
+            const float4 *peers = a.sbuf + (((size_t)par * gridDim.x + (size_t)cl * M) * 8) * RNT + tid;
+#pragma unroll
+            for (int j = 0; j < 8; ++j) {
+                const float4 am = __ldg(ampv + j * RNT);
+                float4 S = make_float4(0.f, 0.f, 0.f, 0.f);
+#pragma unroll
+                for (int mm = 0; mm < (MT ? MT : 8); ++mm) {
+                    if (mm < M) {
+                        float4 v;
+                        if (mm == m) v = make_float4(abs2_rn(u[4 * j]), abs2_rn(u[4 * j + 1]), abs2_rn(u[4 * j + 2]), abs2_rn(u[4 * j + 3]));
+                        else v = __ldcg(peers + ((size_t)mm * 8 + j) * RNT);
+                        S.x += v.x; S.y += v.y; S.z += v.z; S.w += v.w;
+                    }
+                }
+                const float Sv[4] = {S.x, S.y, S.z, S.w}, av[4] = {am.x, am.y, am.z, am.w};
+#pragma unroll
+                for (int c = 0; c < 4; ++c) {
+                    const float rs = rsqrtf(Sv[c] + a.eps);
+                    const float d = Sv[c] * rs - av[c];
+                    e0 = fmaf(d, d, e0);
+                    e1 = fmaf(av[c], av[c], e1);
+                    const float sc = av[c] * rs * cfac;
+                    u[4 * j + c].x *= sc;
+                    u[4 * j + c].y *= sc;
+                }
+            }
+        }
+        // ---- S5: inverse 2-D FFT (mirror) ----
+        pass3<true>(u);
+#pragma unroll
+        for (int z = 0; z < 2; ++z) {
+            __syncthreads();
+            x2_write(u, z, w, t, xb2);
+            __syncthreads();
+            x2_read(u, z, w, t, xb2);
+        }
+        pass2<true>(u);
+        __syncthreads();
+#pragma unroll
+        for (int rho = 0; rho < 2; ++rho) {
+            x1_write(u, rho, t, wbuf);
+            __syncwarp();
+            x1_read(u, rho, t, wbuf);
+            __syncwarp();
+        }
+        {
+            float2 wy[8], wx[4];
+#pragma unroll
+            for (int q = 0; q < 8; ++q) wy[q] = s_wy[w * 8 + q];
+#pragma unroll
+            for (int r = 0; r < 4; ++r) wx[r] = s_wx[t * 4 + r];
+            pass1_inv(u, wy, wx);
+        }
+        // ---- S6: psi_new = psi_old + beta (G - P O) ----
+#pragma unroll
+        for (int r = 0; r < 32; ++r) {
+            float2 *q = psi_f + (r >> 2) * 16 * RN + (r & 3) * 32;
+            const float2 old = *q, po = pobuf[r * RNT + tid];
+            const float tx = u[r].x - po.x, ty = u[r].y - po.y;
+            const float2 nw = make_float2(fmaf(a.beta, tx, old.x), fmaf(a.beta, ty, old.y));
+            e2 = fmaf(tx, tx, fmaf(ty, ty, e2));
+            e3 = fmaf(nw.x, nw.x, fmaf(nw.y, nw.y, e3));
+            *q = nw;
+        }
+    }
+    float acc[4] = {m == 0 ? e0 : 0.f, m == 0 ? e1 : 0.f, e2 * a.beta * a.beta, e3};
+    // deterministic block sum (xor tree in each warp, warps in order)
+#pragma unroll
+    for (int i = 0; i < 4; ++i)
+#pragma unroll
+        for (int s = 16; s > 0; s >>= 1) acc[i] += __shfl_xor_sync(0xffffffffu, acc[i], s);
+    if (t == 0)
+#pragma unroll
+        for (int i = 0; i < 4; ++i) red[i * 32 + w] = acc[i];
+    __syncthreads();
+    if (tid < 4) {
+        float s = 0.f;
+        for (int ww = 0; ww < 16; ++ww) s += red[tid * 32 + ww];
+        a.part[(size_t)blockIdx.x * 4 + tid] = s;
+    }
+}
+
+} // namespace dmreg
+#endif // __CUDACC__

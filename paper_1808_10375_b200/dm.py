@@ -24,7 +24,7 @@ SYMBOLS = (
     "dm_plan_create", "dm_plan_set_param", "dm_plan_workspace_bytes", "dm_plan_set_workspace",
     "dm_set_data", "dm_iterate", "dm_get_probe", "dm_get_object", "dm_get_psi", "dm_get_errors",
     "dm_set_state", "dm_get_window_table", "dm_get_coverage", "dm_get_alphas", "dm_solve_host",
-    "dm_plan_info", "dm_plan_set_profiling", "dm_get_phase_ms", "dm_host_fft2", "dm_status_string", "dm_last_error", "dm_plan_destroy",
+    "dm_plan_info", "dm_plan_set_profiling", "dm_get_phase_ms", "dm_host_fft2", "dm_host_fft2_path", "dm_status_string", "dm_last_error", "dm_plan_destroy",
 )
 
 _vp, _int, _dbl = C.c_void_p, C.c_int, C.c_double
@@ -64,6 +64,7 @@ def lib() -> C.CDLL:
         L.dm_plan_set_profiling.argtypes = [_vp, _int]
         L.dm_get_phase_ms.argtypes = [_vp, _vp, C.POINTER(_int)]
         L.dm_host_fft2.argtypes = [_int, _vp, _vp, _int]
+        L.dm_host_fft2_path.argtypes = [_int, _int, _vp, _vp, _int]
         L.dm_status_string.argtypes = [_int]
         L.dm_status_string.restype = C.c_char_p
         L.dm_last_error.argtypes = [_vp]
@@ -81,11 +82,14 @@ def _np_ptr(a: np.ndarray):
     return a.ctypes.data_as(_vp)
 
 
-def host_fft2(x: np.ndarray, inverse: bool = False) -> np.ndarray:
-    """dm_host_fft2: the kernels' own FFT pass code run on the host (test hook, no CUDA)."""
+def host_fft2(x: np.ndarray, inverse: bool = False, path: int = 0) -> np.ndarray:
+    """dm_host_fft2[_path]: the kernels' own FFT pass code run on the host (test hook, no CUDA)."""
     x = np.ascontiguousarray(x, np.complex64)
     out = np.empty_like(x)
-    st = lib().dm_host_fft2(x.shape[-1], _np_ptr(x), _np_ptr(out), int(inverse))
+    if path:
+        st = lib().dm_host_fft2_path(x.shape[-1], path, _np_ptr(x), _np_ptr(out), int(inverse))
+    else:
+        st = lib().dm_host_fft2(x.shape[-1], _np_ptr(x), _np_ptr(out), int(inverse))
     if st != DM_OK:
         raise DMError(st, "dm_host_fft2")
     return out

@@ -133,3 +133,23 @@ def test_kernel_fft_pass_code_on_host(dm, N, rng):
     u = np.arange(N)
     want = np.exp(-2j * np.pi * (3 * u[:, None] + 5 * u[None, :]) / N)
     assert np.abs(Fd - want).max() < 1e-5
+
+
+def test_register_resident_fft_code_on_host(dm, rng):
+    """Path 3 (csrc/dm_regfft.cuh): the register passes, both exchange layouts (32 x 32 in-warp
+    transpose in two padded rounds, 16 x 16 cross-warp transpose with a staying bit) and the
+    spectrum-layout table, emulated for 512 threads on the host, against the oracle FFT."""
+    N = 128
+    x = (rng.standard_normal((N, N)) + 1j * rng.standard_normal((N, N))).astype(np.complex64)
+    F = dm.host_fft2(x, path=3)
+    Fo = oracle.fft2(x.astype(np.complex128))
+    assert synth.rel_l2(F, Fo) < 2e-6
+    xi = dm.host_fft2(Fo.astype(np.complex64), inverse=True, path=3)
+    assert synth.rel_l2(xi, x) < 2e-6
+    d = np.zeros((N, N), np.complex64)
+    d[7, 33] = 1
+    u = np.arange(N)
+    want = np.exp(-2j * np.pi * (7 * u[:, None] + 33 * u[None, :]) / N)
+    assert np.abs(dm.host_fft2(d, path=3) - want).max() < 1e-5
+    with pytest.raises(dm.DMError):
+        dm.host_fft2(np.zeros((64, 64), np.complex64), path=3)

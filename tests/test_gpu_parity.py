@@ -64,10 +64,15 @@ def forced_pair(dm, pr, t_state, **params):
 
 
 @pytest.mark.parametrize("cfg_i,ny,nx", SMALL)
-@pytest.mark.parametrize("path", [0, 1])
+@pytest.mark.parametrize("path", [0, 1, 2, 3])
 def test_one_iteration_parity(dm, cfg_i, ny, nx, path):
     """P2: set_data state (psi = P0*O0, frozen alphas) is exact; then one full iteration from an
-    identical on-trajectory state (oracle state after 1 iteration) within 1e-5 on psi, P, O."""
+    identical on-trajectory state (oracle state after 1 iteration) within 1e-5 on psi, P, O.
+    path 0 = what dm_iterate picks (register-resident kernel for N = 128, fused shared-memory
+    kernel for N = 64, staged path above); 1, 2, 3 force the staged / fused / register path."""
+    N = synth.CONFIGS[cfg_i].N
+    if (path == 2 and N > 128) or (path == 3 and N != 128):
+        pytest.skip("path not defined for this frame size")
     pr = synth.make_problem(synth.CONFIGS[cfg_i].scaled(ny, nx))
     g, o = make_pair(dm, pr, path=path)
     compare_state(g, o, 1e-6, "t=0")                         # psi init is one complex multiply
