@@ -327,18 +327,29 @@ dm_status launch_object(dm_plan *plan, cudaStream_t st, const float2 *P, const f
                         float *den_out)
 {
     const int tiles = plan->nty * plan->ntx;
-#define OBJ_LAUNCH(LT)                                                                              \
-    object_gather_kernel<LT><<<tiles, OBJ_NT, 0, st>>>(plan->N, plan->K, plan->H, plan->W, plan->pos_d, \
+#define OBJ_LAUNCH(KT, LT)                                                                          \
+    object_gather_kernel<KT, LT><<<tiles, OBJ_NT, 0, st>>>(plan->N, plan->K, plan->H, plan->W, plan->pos_d, \
         plan->tile_ptr_d, plan->tile_views_d, P, plan->psi, O_old, O_new, plan->alphas, plan->partO, den_out)
-    switch (plan->L) {
-    case 1: OBJ_LAUNCH(1); break;
-    case 2: OBJ_LAUNCH(2); break;
-    case 3: OBJ_LAUNCH(3); break;
-    case 4: OBJ_LAUNCH(4); break;
-    case 5: OBJ_LAUNCH(5); break;
-    case 6: OBJ_LAUNCH(6); break;
-    case 7: OBJ_LAUNCH(7); break;
-    default: OBJ_LAUNCH(8); break;
+    const int KL = plan->K * 16 + plan->L;
+    switch (KL) {
+    case 1 * 16 + 1: OBJ_LAUNCH(1, 1); break;
+    case 2 * 16 + 1: OBJ_LAUNCH(2, 1); break;
+    case 3 * 16 + 1: OBJ_LAUNCH(3, 1); break;
+    case 4 * 16 + 1: OBJ_LAUNCH(4, 1); break;
+    case 1 * 16 + 2: OBJ_LAUNCH(1, 2); break;
+    case 2 * 16 + 2: OBJ_LAUNCH(2, 2); break;
+    case 4 * 16 + 2: OBJ_LAUNCH(4, 2); break;
+    default:
+        switch (plan->L) {
+        case 1: OBJ_LAUNCH(0, 1); break;
+        case 2: OBJ_LAUNCH(0, 2); break;
+        case 3: OBJ_LAUNCH(0, 3); break;
+        case 4: OBJ_LAUNCH(0, 4); break;
+        case 5: OBJ_LAUNCH(0, 5); break;
+        case 6: OBJ_LAUNCH(0, 6); break;
+        case 7: OBJ_LAUNCH(0, 7); break;
+        default: OBJ_LAUNCH(0, 8); break;
+        }
     }
 #undef OBJ_LAUNCH
     CU(cudaGetLastError());
@@ -363,7 +374,7 @@ dm_status launch_probe(dm_plan *plan, cudaStream_t st, const float2 *O, const fl
     default: PRB_LAUNCH(8); break;
     }
 #undef PRB_LAUNCH
-    probe_finalize_kernel<<<plan->fin_blocks, 256, 0, st>>>(plan->N, plan->K, plan->prb_chunks, plan->pnum, plan->pden,
+    probe_finalize_kernel<<<dim3((unsigned)plan->fin_blocks, (unsigned)plan->K), 256, 0, st>>>(plan->N, plan->K, plan->prb_chunks, plan->pnum, plan->pden,
                                                             P_old, P_new, plan->alphas, plan->partP, den_out);
     CU(cudaGetLastError());
     return DM_OK;

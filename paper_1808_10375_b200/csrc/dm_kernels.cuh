@@ -351,9 +351,13 @@ __global__ void __launch_bounds__(NT) rows_inv_kernel(const PsiArgs a)
 //   O_new = (alpha O_old + num) / (alpha + den)   (alpha + den == 0: keep O_old)
 constexpr int OBJ_TH = 8, OBJ_TW = 32, OBJ_NT = OBJ_TH * OBJ_TW, OBJ_LMAX = 8;
 
-template <int LT>
+// KT = compile-time K (0: run-time K).  With KT > 0 the covering views are processed in batches
+// of U = 8 / (KT LT) views whose psi and P loads are all issued before the first use (memory-level
+// parallelism); a view that does not contain the pixel contributes exact zeros, so the sum and
+// its order are those of the definition.
+template <int KT, int LT>
 __global__ void __launch_bounds__(OBJ_NT) object_gather_kernel(
-    int N, int K, int H, int W, const int2 *__restrict__ pos, const int *__restrict__ tile_ptr,
+    int N, int K_rt, int H, int W, const int2 *__restrict__ pos, const int *__restrict__ tile_ptr,
     const int *__restrict__ tile_views, const float2 *__restrict__ P, const float2 *__restrict__ psi,
     const float2 *__restrict__ O_old, float2 *__restrict__ O_new, const float *__restrict__ alphas,
     float *__restrict__ part /* [tiles][LT][2] */, float *__restrict__ den_out /* may be NULL */)
@@ -361,6 +365,7 @@ __global__ void __launch_bounds__(OBJ_NT) object_gather_kernel(
     __shared__ int s_j[OBJ_NT];
     __shared__ int2 s_p[OBJ_NT];
     __shared__ float red[2 * LT * 32];
+    const int K = KT ? KT : K_rt;
     const int NN = N * N;
     const int ntx = (W + OBJ_TW - 1) / OBJ_TW;
     const int tile = blockIdx.x, ty = tile / ntx, tx = tile % ntx;
@@ -371,6 +376,7 @@ __global__ void __launch_bounds__(OBJ_NT) object_gather_kernel(
 #pragma unroll
     for (int l = 0; l < LT; ++l) num[l] = make_float2(0.f, 0.f);
     const int beg = tile_ptr[tile], end = tile_ptr[tile + 1];
+    const size_t vstride = (size_t)K * LT * NN;
     for (int b0 = beg; b0 < end; b0 += OBJ_NT) {
         const int nb = min(OBJ_NT, end - b0);
         __syncthreads();
@@ -380,22 +386,55 @@ __global__ void __launch_bounds__(OBJ_NT) object_gather_kernel(
             s_p[threadIdx.x] = pos[j];
         }
         __syncthreads();
-        if (inb) {
-#pragma unroll 4
-            for (int i = 0; i < nb; ++i) {
-                const int ry = y - s_p[i].x, rx = x - s_p[i].y;
-                if ((unsigned)ry < (unsigned)N && (unsigned)rx < (unsigned)N) {
-                    const int r = ry * N + rx;
-                    const float2 *ps = psi + (size_t)s_j[i] * K * LT * NN + r;
-                    for (int k = 0; k < K; ++k) {
-                        const float2 p = __ldg(P + (size_t)k * NN + r);
+        if (!inb) continue;
+        int i = 0;
+        if (KT > 0) {
+            constexpr int KK = KT > 0 ? KT : 1;
+            constexpr int U = (8 / (KK * LT)) > 0 ? (8 / (KK * LT)) : 1;
+            for (; i + U <= nb; i += U) {
+                float2 pv[U][KK], sv[U][KK][LT];
+#pragma unroll
+                for (int u = 0; u < U; ++u) {
+                    const int ry = y - s_p[i + u].x, rx = x - s_p[i + u].y;
+                    const bool ok = (unsigned)ry < (unsigned)N && (unsigned)rx < (unsigned)N;
+                    const int r = ok ? ry * N + rx : 0;
+                    const float2 *ps = psi + (size_t)s_j[i + u] * vstride + r;
+#pragma unroll
+                    for (int k = 0; k < KK; ++k) {
+                        pv[u][k] = ok ? __ldg(P + (size_t)k * NN + r) : make_float2(0.f, 0.f);
+#pragma unroll
+                        for (int l = 0; l < LT; ++l)
+                            sv[u][k][l] = ok ? __ldg(ps + (size_t)(k * LT + l) * NN) : make_float2(0.f, 0.f);
+                    }
+                }
+#pragma unroll
+                for (int u = 0; u < U; ++u)
+#pragma unroll
+                    for (int k = 0; k < KK; ++k) {
+                        const float2 p = pv[u][k];
                         den += cabs2(p);
 #pragma unroll
                         for (int l = 0; l < LT; ++l) {
-                            const float2 s = __ldg(ps + (size_t)(k * LT + l) * NN);
-                            num[l].x += p.x * s.x + p.y * s.y;
-                            num[l].y += p.x * s.y - p.y * s.x;
+                            const float2 sx = sv[u][k][l];
+                            num[l].x += p.x * sx.x + p.y * sx.y;
+                            num[l].y += p.x * sx.y - p.y * sx.x;
                         }
+                    }
+            }
+        }
+        for (; i < nb; ++i) {
+            const int ry = y - s_p[i].x, rx = x - s_p[i].y;
+            if ((unsigned)ry < (unsigned)N && (unsigned)rx < (unsigned)N) {
+                const int r = ry * N + rx;
+                const float2 *ps = psi + (size_t)s_j[i] * vstride + r;
+                for (int k = 0; k < K; ++k) {
+                    const float2 p = __ldg(P + (size_t)k * NN + r);
+                    den += cabs2(p);
+#pragma unroll
+                    for (int l = 0; l < LT; ++l) {
+                        const float2 sx = __ldg(ps + (size_t)(k * LT + l) * NN);
+                        num[l].x += p.x * sx.x + p.y * sx.y;
+                        num[l].y += p.x * sx.y - p.y * sx.x;
                     }
                 }
             }
@@ -471,6 +510,7 @@ __global__ void __launch_bounds__(PRB_NT) probe_partial_kernel(
 }
 
 // stage 2: fixed-order (chunk ascending) FP64 sum of the partials, inertial quotient, eq. (7) partials.
+// grid = (pixel blocks, K): one probe mode per blockIdx.y (the shared denominator is re-summed per mode).
 __global__ void __launch_bounds__(256) probe_finalize_kernel(
     int N, int K, int C, const float2 *__restrict__ pnum, const float *__restrict__ pden,
     const float2 *__restrict__ P_old, float2 *__restrict__ P_new, const float *__restrict__ alphas,
@@ -479,34 +519,47 @@ __global__ void __launch_bounds__(256) probe_finalize_kernel(
     __shared__ float red[2 * 32];
     const int NN = N * N;
     const int r = blockIdx.x * blockDim.x + threadIdx.x;
+    const int k = blockIdx.y;
     const bool inb = r < NN;
-    double den = 0.0;
-    if (inb) for (int c = 0; c < C; ++c) den += (double)pden[(size_t)c * NN + r];
-    const float alpha = alphas[1];
-    const float denf = (float)den, dd = alpha + denf;
-    if (inb && den_out) den_out[r] = denf;
-    for (int k = 0; k < K; ++k) {
-        float acc[2] = {0.f, 0.f};
-        if (inb) {
-            double nx = 0.0, ny = 0.0;
-            for (int c = 0; c < C; ++c) {
-                const float2 v = pnum[((size_t)c * K + k) * NN + r];
-                nx += (double)v.x;
-                ny += (double)v.y;
+    float acc[2] = {0.f, 0.f};
+    if (inb) {
+        double den = 0.0, nx = 0.0, ny = 0.0;
+        int c = 0;
+        for (; c + 8 <= C; c += 8) {
+            float d[8];
+            float2 v[8];
+#pragma unroll
+            for (int u = 0; u < 8; ++u) {
+                d[u] = pden[(size_t)(c + u) * NN + r];
+                v[u] = pnum[((size_t)(c + u) * K + k) * NN + r];
             }
-            const float2 po = P_old[(size_t)k * NN + r];
-            float2 pn = po;
-            if (dd > 0.f) pn = make_float2((alpha * po.x + (float)nx) / dd, (alpha * po.y + (float)ny) / dd);
-            P_new[(size_t)k * NN + r] = pn;
-            acc[0] = cabs2(csub(pn, po));
-            acc[1] = cabs2(pn);
+#pragma unroll
+            for (int u = 0; u < 8; ++u) {
+                den += (double)d[u];
+                nx += (double)v[u].x;
+                ny += (double)v[u].y;
+            }
         }
-        block_sum<2>(acc, red);
-        if (threadIdx.x == 0) {
-            part[((size_t)blockIdx.x * K + k) * 2] = acc[0];
-            part[((size_t)blockIdx.x * K + k) * 2 + 1] = acc[1];
+        for (; c < C; ++c) {
+            den += (double)pden[(size_t)c * NN + r];
+            const float2 v = pnum[((size_t)c * K + k) * NN + r];
+            nx += (double)v.x;
+            ny += (double)v.y;
         }
-        __syncthreads();
+        const float alpha = alphas[1];
+        const float denf = (float)den, dd = alpha + denf;
+        if (den_out && k == 0) den_out[r] = denf;
+        const float2 po = P_old[(size_t)k * NN + r];
+        float2 pn = po;
+        if (dd > 0.f) pn = make_float2((alpha * po.x + (float)nx) / dd, (alpha * po.y + (float)ny) / dd);
+        P_new[(size_t)k * NN + r] = pn;
+        acc[0] = cabs2(csub(pn, po));
+        acc[1] = cabs2(pn);
+    }
+    block_sum<2>(acc, red);
+    if (threadIdx.x == 0) {
+        part[((size_t)blockIdx.x * K + k) * 2] = acc[0];
+        part[((size_t)blockIdx.x * K + k) * 2 + 1] = acc[1];
     }
 }
 
