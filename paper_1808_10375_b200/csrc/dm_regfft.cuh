@@ -249,9 +249,36 @@ struct RegArgs {
     float beta, eps;
 };
 
-constexpr int REG_SMEM_V1 = XBUF_BYTES + RNN * 8 + 2048;     // exchange + P*O + twiddles
+constexpr int REG_SMEM_V1 = XBUF_BYTES + 2048;               // exchange buffer + twiddles
 
 __device__ __forceinline__ float abs2_rn(float2 f) { return __fmaf_rn(f.y, f.y, __fmul_rn(f.x, f.x)); }
+
+// ---- tensor memory as a per-thread spill space ---------------------------------------------
+// TMEM (256 KiB per SM, 128 lanes x 512 32-bit columns) is otherwise idle in this kernel (no
+// tensor-core work).  The 32x32b shape maps lane i of a warp to TMEM lane 32 (warp % 4) + i, so a
+// column range is private to a thread: psi_old and P*O of the frame (64 words each per thread)
+// are parked there during the FFTs instead of being re-read from L2 / kept in shared memory.
+__device__ __forceinline__ void tmem_st8(uint32_t taddr, float2 a, float2 b, float2 c, float2 d)
+{
+    asm volatile("tcgen05.st.sync.aligned.32x32b.x8.b32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8};\n"
+                 :: "r"(taddr), "r"(__float_as_uint(a.x)), "r"(__float_as_uint(a.y)), "r"(__float_as_uint(b.x)),
+                    "r"(__float_as_uint(b.y)), "r"(__float_as_uint(c.x)), "r"(__float_as_uint(c.y)),
+                    "r"(__float_as_uint(d.x)), "r"(__float_as_uint(d.y)) : "memory");
+}
+__device__ __forceinline__ void tmem_ld8(uint32_t taddr, float2 &a, float2 &b, float2 &c, float2 &d)
+{
+    uint32_t r0, r1, r2, r3, r4, r5, r6, r7;
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0, %1, %2, %3, %4, %5, %6, %7}, [%8];\n"
+                 : "=r"(r0), "=r"(r1), "=r"(r2), "=r"(r3), "=r"(r4), "=r"(r5), "=r"(r6), "=r"(r7) : "r"(taddr) : "memory");
+    a = make_float2(__uint_as_float(r0), __uint_as_float(r1));
+    b = make_float2(__uint_as_float(r2), __uint_as_float(r3));
+    c = make_float2(__uint_as_float(r4), __uint_as_float(r5));
+    d = make_float2(__uint_as_float(r6), __uint_as_float(r7));
+}
+__device__ __forceinline__ void tmem_wait_st() { asm volatile("tcgen05.wait::st.sync.aligned;\n" ::: "memory"); }
+__device__ __forceinline__ void tmem_wait_ld() { asm volatile("tcgen05.wait::ld.sync.aligned;\n" ::: "memory"); }
+__device__ __forceinline__ void cluster_arrive() { asm volatile("barrier.cluster.arrive.release.aligned;\n" ::: "memory"); }
+__device__ __forceinline__ void cluster_wait() { asm volatile("barrier.cluster.wait.acquire.aligned;\n" ::: "memory"); }
 
 // Persistent CTAs; cluster = the M = K*L mode frames of one view (cluster rank m = mode index),
 // cluster c processes views c, c + n_clusters, ...  MT = compile-time M (0: run-time M).
@@ -261,10 +288,10 @@ __global__ void __launch_bounds__(RNT, 1) regfft128_kernel(const RegArgs a)
     namespace cg = cooperative_groups;
     extern __shared__ __align__(16) unsigned char smem[];
     unsigned char *xbuf = smem;
-    float2 *pobuf = reinterpret_cast<float2 *>(smem + XBUF_BYTES);
-    float2 *s_wy = reinterpret_cast<float2 *>(smem + XBUF_BYTES + RNN * 8);
+    float2 *s_wy = reinterpret_cast<float2 *>(smem + XBUF_BYTES);
     float2 *s_wx = s_wy + 128;
     __shared__ float red[4 * 32];
+    __shared__ uint32_t s_tmem;
 
     const int tid = threadIdx.x, w = tid >> 5, t = tid & 31;
     const int M = MT ? MT : a.K * a.L;
@@ -272,7 +299,17 @@ __global__ void __launch_bounds__(RNT, 1) regfft128_kernel(const RegArgs a)
     const int k = m / a.L, l = m % a.L;
     if (tid < 128) s_wy[tid] = a.wy[tid];
     else if (tid < 256) s_wx[tid - 128] = a.wx[tid - 128];
+    if (w == 0) {       // all 512 TMEM columns (this kernel is the only resident CTA of its SM)
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;\n"
+                     :: "r"((uint32_t)__cvta_generic_to_shared(&s_tmem)), "r"(512) : "memory");
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;\n" ::: "memory");
+    }
+    asm volatile("tcgen05.fence::before_thread_sync;\n" ::: "memory");
     __syncthreads();
+    asm volatile("tcgen05.fence::after_thread_sync;\n" ::: "memory");
+    // this thread's private columns: lane quarter w % 4, column block (w / 4) * 128; psi_old | P*O
+    const uint32_t t_psi = s_tmem + ((uint32_t)(32 * (w & 3)) << 16) + (uint32_t)(w >> 2) * 128u;
+    const uint32_t t_po = t_psi + 64u;
 
     unsigned char *wbuf = xbuf + w * X1_WARP;
     float2 *xb2 = reinterpret_cast<float2 *>(xbuf);
@@ -286,7 +323,7 @@ __global__ void __launch_bounds__(RNT, 1) regfft128_kernel(const RegArgs a)
         float2 *psi_f = a.psi + ((size_t)view * M + m) * RNN + w * RN + t;
         const float2 *Ow = a.O + (size_t)l * a.H * a.W + (size_t)(p0.x + w) * a.W + p0.y + t;
         float2 u[32];
-        // ---- S1 + S2: R = 2 P O - psi in L0; P*O parked in shared memory ----
+        // ---- S1 + S2: R = 2 P O - psi in L0; psi_old and P*O parked in tensor memory ----
 #pragma unroll
         for (int r = 0; r < 32; ++r) u[r] = psi_f[(r >> 2) * 16 * RN + (r & 3) * 32];
 #pragma unroll
@@ -297,13 +334,16 @@ __global__ void __launch_bounds__(RNT, 1) regfft128_kernel(const RegArgs a)
                 p[r] = __ldg(Pk + i * 16 * RN + r * 32);
                 o[r] = __ldg(Ow + (size_t)i * 16 * a.W + r * 32);
             }
+            tmem_st8(t_psi + 8 * i, u[4 * i], u[4 * i + 1], u[4 * i + 2], u[4 * i + 3]);
+            float2 po[4];
 #pragma unroll
             for (int r = 0; r < 4; ++r) {
-                const float2 po = cmul(p[r], o[r]);
-                pobuf[(4 * i + r) * RNT + tid] = po;
-                u[4 * i + r] = make_float2(2.f * po.x - u[4 * i + r].x, 2.f * po.y - u[4 * i + r].y);
+                po[r] = cmul(p[r], o[r]);
+                u[4 * i + r] = make_float2(2.f * po[r].x - u[4 * i + r].x, 2.f * po[r].y - u[4 * i + r].y);
             }
+            tmem_st8(t_po + 8 * i, po[0], po[1], po[2], po[3]);
         }
+        tmem_wait_st();
         // ---- S3: forward 2-D FFT ----
         {
             float2 wy[8], wx[4];
@@ -336,7 +376,8 @@ __global__ void __launch_bounds__(RNT, 1) regfft128_kernel(const RegArgs a)
 #pragma unroll
                 for (int j = 0; j < 8; ++j)
                     mine[j * RNT] = make_float4(abs2_rn(u[4 * j]), abs2_rn(u[4 * j + 1]), abs2_rn(u[4 * j + 2]), abs2_rn(u[4 * j + 3]));
-                cg::this_cluster().sync();
+                cluster_arrive();
+                cluster_wait();
             } else {
                 __syncthreads();
             }
@@ -396,16 +437,27 @@ __global__ void __launch_bounds__(RNT, 1) regfft128_kernel(const RegArgs a)
         }
         // ---- S6: psi_new = psi_old + beta (G - P O) ----
 #pragma unroll
-        for (int r = 0; r < 32; ++r) {
-            float2 *q = psi_f + (r >> 2) * 16 * RN + (r & 3) * 32;
-            const float2 old = *q, po = pobuf[r * RNT + tid];
-            const float tx = u[r].x - po.x, ty = u[r].y - po.y;
-            const float2 nw = make_float2(fmaf(a.beta, tx, old.x), fmaf(a.beta, ty, old.y));
-            e2 = fmaf(tx, tx, fmaf(ty, ty, e2));
-            e3 = fmaf(nw.x, nw.x, fmaf(nw.y, nw.y, e3));
-            *q = nw;
+        for (int i = 0; i < 8; i += 2) {
+            float2 old[8], po[8];
+            tmem_ld8(t_psi + 8 * i, old[0], old[1], old[2], old[3]);
+            tmem_ld8(t_psi + 8 * i + 8, old[4], old[5], old[6], old[7]);
+            tmem_ld8(t_po + 8 * i, po[0], po[1], po[2], po[3]);
+            tmem_ld8(t_po + 8 * i + 8, po[4], po[5], po[6], po[7]);
+            tmem_wait_ld();
+#pragma unroll
+            for (int r = 0; r < 8; ++r) {
+                const int e = 4 * i + r;
+                const float tx = u[e].x - po[r].x, ty = u[e].y - po[r].y;
+                const float2 nw = make_float2(fmaf(a.beta, tx, old[r].x), fmaf(a.beta, ty, old[r].y));
+                e2 = fmaf(tx, tx, fmaf(ty, ty, e2));
+                e3 = fmaf(nw.x, nw.x, fmaf(nw.y, nw.y, e3));
+                psi_f[(e >> 2) * 16 * RN + (e & 3) * 32] = nw;
+            }
         }
     }
+    asm volatile("tcgen05.fence::before_thread_sync;\n" ::: "memory");
+    __syncthreads();
+    if (w == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;\n" :: "r"(s_tmem), "r"(512) : "memory");
     float acc[4] = {m == 0 ? e0 : 0.f, m == 0 ? e1 : 0.f, e2 * a.beta * a.beta, e3};
     // deterministic block sum (xor tree in each warp, warps in order)
 #pragma unroll
