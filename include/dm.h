@@ -55,10 +55,16 @@ typedef enum {
     DM_PARAM_ALPHA_OBJ = 1,   /* relative inertial factor a_O >= 0 of eq. (6); default 1e-3  */
     DM_PARAM_ALPHA_PROBE = 2, /* relative inertial factor a_P >= 0 of eq. (5); default 1e-3  */
     DM_PARAM_EPS_F = 3,       /* zero guard in eq. (4): scale = amp/sqrt(S+eps); default 1e-30 */
-    DM_PARAM_PATH = 4         /* 0 = auto (default), 1 = force the staged (L2-scratch) path,
+    DM_PARAM_PATH = 4,        /* 0 = auto (default), 1 = force the staged (L2-scratch) path,
                                  2 = force the fused shared-memory path (DM_ERR_UNSUPPORTED at
                                  dm_set_data if N > 128), 3 = force the register-resident
-                                 path (DM_ERR_UNSUPPORTED at dm_set_data unless N = 128)     */
+                                 path (DM_ERR_UNSUPPORTED at dm_set_data unless N = 128),
+                                 4 = force the view-pipelined warp-FFT path (any N; the
+                                 default for N >= 256)                                       */
+    DM_PARAM_LAG = 5          /* path 4: views between the row, column and inverse-row phases
+                                 of one view (integer >= 1; 0 = derive from the task counts,
+                                 default).  Sizes the scratch ring: set before
+                                 dm_plan_set_workspace (INVALID_ARG afterwards)              */
 } dm_param;
 
 /* Build the plan (HOST only, no CUDA call): validates, copies `positions` (HOST,

@@ -37,6 +37,11 @@ struct dm_plan {
     double beta, a_obj, a_probe, eps_f;
     int path_req, path;                  // requested / chosen (1 staged, 2 fused, 3 register-resident)
     int reg_grid;                        // path 3: number of persistent CTAs (multiple of M)
+    // path 4 (dm_warpfft.cuh): ring slots, phase lag (views), tasks per view and phase, persistent CTAs
+    int wf_S, wf_D, wf_nA, wf_nB, wf_nC, wf_grid;
+    int wf_lag_req;                      // 0 = derive the lag from the task counts
+    int *wf_cnt;                         // [1 + 3 n_views] queue counter, cntA, cntB, cntC
+    float2 *wf_tw_d;                     // [N/32][32] stage-1 twiddles
     // probe reduction geometry
     int prb_blocks, prb_chunks, prb_chunk_len, fin_blocks;
     // staged geometry
@@ -139,6 +144,19 @@ void plan_geometry(dm_plan *p)
     if (cv < 1) cv = 1;
     if (cv > (size_t)p->n_views) cv = p->n_views;
     p->chunk_views = (int)cv;
+    // path 4: a CTA task = 8 row groups (phases A, C) or 8 / M column groups x M modes (phase B)
+    const int G = 1024 / p->N, NG = p->N / G, GPT = dmwf::WF_WARPS / p->M;
+    p->wf_nA = (p->M * NG + dmwf::WF_WARPS - 1) / dmwf::WF_WARPS;
+    p->wf_nC = p->wf_nA;
+    p->wf_nB = (NG + GPT - 1) / GPT;
+    const int T = p->wf_nA + p->wf_nB + p->wf_nC;
+    // lag: a phase starts on a view once ~1.2 x (resident CTAs = 2 x 148) tasks have been queued behind its inputs
+    int D = p->wf_lag_req > 0 ? p->wf_lag_req : (int)((1.2 * 296 + T - 1) / T);
+    if (D < 1) D = 1;
+    p->wf_D = D;
+    p->wf_S = 2 * D + 4;
+    if (p->wf_S > p->n_views) p->wf_S = p->n_views;
+    if (p->wf_S <= 2 * D) p->wf_S = 2 * D + 1;       // keeps "A(v) waits for C(v - S)" behind it in the queue
 }
 
 // carve (or, with base == nullptr, just measure) the workspace
@@ -155,6 +173,7 @@ size_t carve(dm_plan *p, unsigned char *base)
     const int rows_tiles = p->N / (4096 / p->N);                         // row tiles per frame (staged)
     p->nA = p->n_views * (p->N / COLS_SW);
     p->nB = (int)(MV * rows_tiles);
+
     p->psi = (float2 *)take(MV * NN * sizeof(float2));
     p->amp = (float *)take((size_t)p->n_views * NN * sizeof(float));
     for (int i = 0; i < 2; ++i) p->Pbuf[i] = (float2 *)take(p->K * NN * sizeof(float2));
@@ -165,8 +184,11 @@ size_t carve(dm_plan *p, unsigned char *base)
     p->alphas = (float *)take(2 * sizeof(float));
     size_t nA = (size_t)p->nA * 2 > MV * 4 ? (size_t)p->nA * 2 : MV * 4;
     if (nA < (size_t)REG_MAX_CTAS * 4) nA = (size_t)REG_MAX_CTAS * 4;
+    if (nA < (size_t)p->n_views * p->wf_nB * 2) nA = (size_t)p->n_views * p->wf_nB * 2;
+    size_t nB = (size_t)p->nB * 2;
+    if (nB < (size_t)p->n_views * p->wf_nC * 2) nB = (size_t)p->n_views * p->wf_nC * 2;
     p->partA = (float *)take(nA * sizeof(float));
-    p->partB = (float *)take((size_t)p->nB * 2 * sizeof(float));
+    p->partB = (float *)take(nB * sizeof(float));
     p->partP = (float *)take((size_t)p->fin_blocks * p->K * 2 * sizeof(float));
     p->partO = (float *)take((size_t)p->nty * p->ntx * p->L * 2 * sizeof(float));
     p->pos_d = (int2 *)take((size_t)p->n_views * sizeof(int2));
@@ -178,7 +200,12 @@ size_t carve(dm_plan *p, unsigned char *base)
     p->sbuf = (float4 *)take(p->N == 128 ? (size_t)2 * REG_MAX_CTAS * 8 * dmreg::RNT * sizeof(float4) : 0);
     p->tw_d = (float2 *)take(p->N * sizeof(float2));
     p->errors = (double *)take((size_t)ERR_ROWS_CAP * (2 + p->K + p->L) * sizeof(double));
-    p->scratch = (float2 *)take((size_t)p->chunk_views * p->M * NN * sizeof(float2));
+    {
+        size_t sc = (size_t)p->chunk_views * p->M * NN, ring = (size_t)p->wf_S * p->M * NN;
+        p->scratch = (float2 *)take((sc > ring ? sc : ring) * sizeof(float2));
+    }
+    p->wf_cnt = (int *)take((1 + 3 * (size_t)p->n_views) * sizeof(int));
+    p->wf_tw_d = (float2 *)take((size_t)p->N * sizeof(float2));
     p->stage_I = (float *)take((size_t)p->n_views * NN * sizeof(float));
     p->stage_P = (float2 *)take(p->K * NN * sizeof(float2));
     p->stage_O = (float2 *)take(p->L * HW * sizeof(float2));
@@ -308,8 +335,55 @@ dm_status launch_regfft(dm_plan *plan, cudaStream_t st, bool query_only)
     }
 }
 
+// path 4: persistent task-queue kernel (rows -> columns + modulus -> rows through an L2-resident ring)
+template <int N> dm_status launch_wf_t(dm_plan *plan, cudaStream_t st, bool query_only)
+{
+    auto kern = dmwf::wf_dataflow_kernel<N>;
+    const int smem = dmwf::WF_WARPS * dmwf::WF_XBUF + dmwf::WF_WARPS * 4096 + (N / 32) * 32 * (int)sizeof(float2);
+    static bool attr_done = false;
+    if (!attr_done) {
+        CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+        attr_done = true;
+    }
+    if (query_only) {
+        int dev = 0, sms = 0, per = 0;
+        CU(cudaGetDevice(&dev));
+        CU(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+        CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per, kern, dmwf::WF_NT, smem));
+        if (per < 1) return fail(plan, DM_ERR_CUDA, "warp-FFT kernel does not fit an SM");
+        plan->wf_grid = sms * per;
+        return DM_OK;
+    }
+    dmwf::WfArgs a;
+    memset(&a, 0, sizeof a);
+    a.n_views = plan->n_views; a.K = plan->K; a.L = plan->L; a.H = plan->H; a.W = plan->W;
+    a.pos = plan->pos_d; a.P = plan->Pbuf[plan->curP]; a.O = plan->Obuf[plan->curO];
+    a.psi = plan->psi; a.amp = plan->amp; a.tw = plan->wf_tw_d; a.scratch = plan->scratch;
+    a.S = plan->wf_S; a.D = plan->wf_D; a.nA = plan->wf_nA; a.nB = plan->wf_nB; a.nC = plan->wf_nC;
+    a.queue = plan->wf_cnt; a.cntA = plan->wf_cnt + 1; a.cntB = a.cntA + plan->n_views; a.cntC = a.cntB + plan->n_views;
+    a.partF = plan->partA; a.partS = plan->partB;
+    a.beta = (float)plan->beta; a.eps = (float)plan->eps_f;
+    CU(cudaMemsetAsync(plan->wf_cnt, 0, (1 + 3 * (size_t)plan->n_views) * sizeof(int), st));
+    const long long tasks = (long long)(plan->n_views + 2 * plan->wf_D) * (plan->wf_nA + plan->wf_nB + plan->wf_nC);
+    const int grid = tasks < plan->wf_grid ? (int)tasks : plan->wf_grid;
+    kern<<<grid, dmwf::WF_NT, smem, st>>>(a);
+    CU(cudaGetLastError());
+    return DM_OK;
+}
+
+dm_status launch_wf(dm_plan *plan, cudaStream_t st, bool query_only)
+{
+    switch (plan->N) {
+    case 64: return launch_wf_t<64>(plan, st, query_only);
+    case 128: return launch_wf_t<128>(plan, st, query_only);
+    case 256: return launch_wf_t<256>(plan, st, query_only);
+    default: return launch_wf_t<512>(plan, st, query_only);
+    }
+}
+
 dm_status launch_psi_update(dm_plan *plan, cudaStream_t st)
 {
+    if (plan->path == 4) return launch_wf(plan, st, false);
     if (plan->path == 3) return launch_regfft(plan, st, false);
     if (plan->path == 2) {
         if (plan->N == 64) return launch_fused<64, 256>(plan, st);
@@ -417,7 +491,7 @@ dm_status dm_plan_create(dm_plan **out, int N, int n_views, int K, int L, int ob
     p->N = N; p->n_views = n_views; p->K = K; p->L = L; p->M = K * L; p->H = obj_h; p->W = obj_w;
     p->pos.assign(positions, positions + 2 * (size_t)n_views);
     p->beta = 1.0; p->a_obj = 1e-3; p->a_probe = 1e-3; p->eps_f = 1e-30;
-    p->path_req = 0; p->path = 0;
+    p->path_req = 0; p->path = 0; p->wf_lag_req = 0;
     p->ws = nullptr; p->ws_bytes = 0;
     p->curP = p->curO = 0; p->has_data = false; p->rows = 0;
     p->profiling = false; p->ev_iters = 0;
@@ -438,7 +512,14 @@ dm_status dm_plan_set_param(dm_plan *plan, dm_param which, double v)
     case DM_PARAM_ALPHA_OBJ: if (v < 0) break; plan->a_obj = v; return DM_OK;
     case DM_PARAM_ALPHA_PROBE: if (v < 0) break; plan->a_probe = v; return DM_OK;
     case DM_PARAM_EPS_F: if (v < 0) break; plan->eps_f = v; return DM_OK;
-    case DM_PARAM_PATH: if (v != 0 && v != 1 && v != 2 && v != 3) break; plan->path_req = (int)v; return DM_OK;
+    case DM_PARAM_PATH: if (v != 0 && v != 1 && v != 2 && v != 3 && v != 4) break; plan->path_req = (int)v; return DM_OK;
+    case DM_PARAM_LAG:
+        if (v < 0 || v > 4096 || v != (double)(int)v) break;
+        if (plan->ws) return fail(plan, DM_ERR_INVALID_ARG, "the phase lag sizes the workspace: set it before dm_plan_set_workspace");
+        plan->wf_lag_req = (int)v;
+        plan_geometry(plan);
+        plan->need_bytes = carve(plan, nullptr);
+        return DM_OK;
     default: return fail(plan, DM_ERR_INVALID_ARG, "unknown parameter %d", (int)which);
     }
     return fail(plan, DM_ERR_INVALID_ARG, "parameter %d: value %g out of range", (int)which, v);
@@ -471,7 +552,7 @@ dm_status dm_set_data(dm_plan *plan, const float *intensities, const float *prob
     if (s != DM_OK) return s;
     if (!intensities || !probe0 || !object0) return fail(plan, DM_ERR_INVALID_ARG, "NULL data pointer");
     int path = plan->path_req;
-    if (path == 0) path = plan->N == 128 ? 3 : (plan->N < 128 ? 2 : 1);
+    if (path == 0) path = plan->N == 128 ? 3 : (plan->N < 128 ? 2 : 4);
     if (path == 2 && plan->N > 128)
         return fail(plan, DM_ERR_UNSUPPORTED, "fused per-frame path needs N <= 128 (N = %d)", plan->N);
     if (path == 3 && plan->N != 128)
@@ -501,6 +582,31 @@ dm_status dm_set_data(dm_plan *plan, const float *intensities, const float *prob
         CU(cudaMemcpyAsync(plan->wx_d, wx.data(), 256 * sizeof(float), cudaMemcpyHostToDevice, st));
         CU(cudaStreamSynchronize(st));          // wy / wx are stack-owned host buffers
         dm_status qs = launch_regfft(plan, st, true);
+        if (qs != DM_OK) return qs;
+    } else if (path == 4) {
+        const int N = plan->N, RX = N / 32, G = 32 / RX;
+        for (int cg = 0; cg < N / G; ++cg)
+            for (int a = 0; a < 32; ++a)
+                for (int k2 = 0; k2 < 32; ++k2) {
+                    int f;
+                    switch (N) {
+                    case 64: f = dmwf::spec_freq<64>(cg, a, k2); break;
+                    case 128: f = dmwf::spec_freq<128>(cg, a, k2); break;
+                    case 256: f = dmwf::spec_freq<256>(cg, a, k2); break;
+                    default: f = dmwf::spec_freq<512>(cg, a, k2); break;
+                    }
+                    plan->spec[dmwf::spec_pos(cg, a, k2)] = f;
+                }
+        std::vector<float> tw((size_t)RX * 32 * 2);
+        for (int k1 = 0; k1 < RX; ++k1)
+            for (int t = 0; t < 32; ++t) {
+                const double ang = -2.0 * M_PI * (double)(t * k1) / (double)N;
+                tw[2 * (k1 * 32 + t)] = (float)std::cos(ang);
+                tw[2 * (k1 * 32 + t) + 1] = (float)std::sin(ang);
+            }
+        CU(cudaMemcpyAsync(plan->wf_tw_d, tw.data(), tw.size() * sizeof(float), cudaMemcpyHostToDevice, st));
+        CU(cudaStreamSynchronize(st));          // tw is a stack-owned host buffer
+        dm_status qs = launch_wf(plan, st, true);
         if (qs != DM_OK) return qs;
     } else {
         for (int py = 0; py < plan->N; ++py)
@@ -566,7 +672,10 @@ dm_status dm_iterate(dm_plan *plan, int n_iter, void *stream)
         if (s != DM_OK) return s;
         if (ev) CU(cudaEventRecord(ev[3], st));
         ErrArgs e;                                                                   // S9
-        if (plan->path == 3) {
+        if (plan->path == 4) {
+            e.pF = plan->partA; e.nF = plan->n_views * plan->wf_nB; e.sF = 2;
+            e.pS = plan->partB; e.nS = plan->n_views * plan->wf_nC; e.sS = 2;
+        } else if (plan->path == 3) {
             e.pF = plan->partA;     e.nF = plan->reg_grid; e.sF = 4;
             e.pS = plan->partA + 2; e.nS = plan->reg_grid; e.sS = 4;
         } else if (plan->path == 2) {
@@ -734,7 +843,7 @@ dm_status dm_get_phase_ms(dm_plan *plan, float *out_ms4, int *iters)
 dm_status dm_plan_info(const dm_plan *plan, int *path, int *launches_per_iter)
 {
     if (!plan) return DM_ERR_INVALID_ARG;
-    int p = plan->path ? plan->path : (plan->path_req ? plan->path_req : (plan->N == 128 ? 3 : (plan->N < 128 ? 2 : 1)));
+    int p = plan->path ? plan->path : (plan->path_req ? plan->path_req : (plan->N == 128 ? 3 : (plan->N < 128 ? 2 : 4)));
     if (path) *path = p;
     if (launches_per_iter) {
         const int chunks = (plan->n_views + plan->chunk_views - 1) / plan->chunk_views;
@@ -834,6 +943,74 @@ void host_fft2_reg(const float *in, float *out, int inverse)
             for (int a = 0; a < REPT; ++a) dst[l0_pixel(tid, a)] = make_float2(U(tid)[a].x * s, U(tid)[a].y * s);
     }
 }
+// path 4 (dm_warpfft.cuh): one emulated warp (32 lanes, phase by phase) per row group / column group
+template <int N> void host_fft2_wf(const float *in, float *out, int inverse)
+{
+    using namespace dmwf;
+    constexpr int RX = N / 32, G = 32 / RX, NG = N / G;
+    std::vector<float2> tw((size_t)RX * 32), scratch((size_t)N * N), regs(32 * 32);
+    std::vector<float4> xbuf_v(WF_XBUF / 16);
+    unsigned char *xbuf = reinterpret_cast<unsigned char *>(xbuf_v.data());
+    for (int k1 = 0; k1 < RX; ++k1)
+        for (int t = 0; t < 32; ++t) {
+            const double ang = -2.0 * M_PI * (double)(t * k1) / (double)N;
+            tw[k1 * 32 + t] = make_float2((float)std::cos(ang), (float)std::sin(ang));
+        }
+    auto U = [&](int lane) -> float2(&)[32] { return *reinterpret_cast<float2(*)[32]>(&regs[(size_t)lane * 32]); };
+    auto exch = [&]() {
+        for (int rho = 0; rho < 2; ++rho) {
+            for (int t = 0; t < 32; ++t) dmreg::x1_write(U(t), rho, t, xbuf);
+            for (int t = 0; t < 32; ++t) dmreg::x1_read(U(t), rho, t, xbuf);
+        }
+    };
+    auto fwd = [&]() {
+        for (int t = 0; t < 32; ++t) stage1_fwd<RX>(U(t), tw.data(), t);
+        exch();
+        for (int t = 0; t < 32; ++t) dmreg::dft32<false>(U(t));
+    };
+    auto inv = [&]() {
+        for (int t = 0; t < 32; ++t) dmreg::dft32<true>(U(t));
+        exch();
+        for (int t = 0; t < 32; ++t) stage1_inv<RX>(U(t), tw.data(), t);
+    };
+    const float2 *src = reinterpret_cast<const float2 *>(in);
+    float2 *dst = reinterpret_cast<float2 *>(out);
+    if (!inverse) {
+        for (int rg = 0; rg < NG; ++rg) {                      // phase A: rows
+            for (int t = 0; t < 32; ++t)
+                for (int i = 0; i < 32; ++i) U(t)[i] = src[(size_t)(rg * G + i / RX) * N + t + 32 * (i % RX)];
+            fwd();
+            for (int a = 0; a < 32; ++a)
+                for (int k2 = 0; k2 < 32; ++k2) scratch[scratch_index<N>(rg * G + a / RX, a % RX + RX * k2)] = U(a)[k2];
+        }
+        for (int cg = 0; cg < NG; ++cg) {                      // phase B: columns
+            for (int t = 0; t < 32; ++t)
+                for (int i = 0; i < 32; ++i) U(t)[i] = scratch[((size_t)cg * N + t + 32 * (i % RX)) * G + i / RX];
+            fwd();
+            for (int a = 0; a < 32; ++a)
+                for (int k2 = 0; k2 < 32; ++k2) dst[spec_freq<N>(cg, a, k2)] = U(a)[k2];
+        }
+    } else {
+        for (int cg = 0; cg < NG; ++cg) {
+            for (int a = 0; a < 32; ++a)
+                for (int k2 = 0; k2 < 32; ++k2) U(a)[k2] = src[spec_freq<N>(cg, a, k2)];
+            inv();
+            for (int t = 0; t < 32; ++t)
+                for (int i = 0; i < 32; ++i) scratch[((size_t)cg * N + t + 32 * (i % RX)) * G + i / RX] = U(t)[i];
+        }
+        const float sc = 1.f / ((float)N * (float)N);
+        for (int rg = 0; rg < NG; ++rg) {
+            for (int a = 0; a < 32; ++a)
+                for (int k2 = 0; k2 < 32; ++k2) U(a)[k2] = scratch[scratch_index<N>(rg * G + a / RX, a % RX + RX * k2)];
+            inv();
+            for (int t = 0; t < 32; ++t)
+                for (int i = 0; i < 32; ++i) {
+                    const float2 v = U(t)[i];
+                    dst[(size_t)(rg * G + i / RX) * N + t + 32 * (i % RX)] = make_float2(v.x * sc, v.y * sc);
+                }
+        }
+    }
+}
 } // namespace
 
 extern "C" {
@@ -844,6 +1021,16 @@ dm_status dm_host_fft2_path(int N, int path, const float *in_host, float *out_ho
     if (path == 3) {
         if (N != 128) return DM_ERR_UNSUPPORTED;
         host_fft2_reg(in_host, out_host, inverse);
+        return DM_OK;
+    }
+    if (path == 4) {
+        switch (N) {
+        case 64: host_fft2_wf<64>(in_host, out_host, inverse); break;
+        case 128: host_fft2_wf<128>(in_host, out_host, inverse); break;
+        case 256: host_fft2_wf<256>(in_host, out_host, inverse); break;
+        case 512: host_fft2_wf<512>(in_host, out_host, inverse); break;
+        default: return DM_ERR_UNSUPPORTED;
+        }
         return DM_OK;
     }
     if (path != 1 && path != 2) return DM_ERR_INVALID_ARG;

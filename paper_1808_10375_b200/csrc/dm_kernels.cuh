@@ -17,6 +17,7 @@
 
 #include "dm_fft.cuh"
 #include "dm_regfft.cuh"
+#include "dm_warpfft.cuh"
 
 namespace cg = cooperative_groups;
 using namespace dmfft;

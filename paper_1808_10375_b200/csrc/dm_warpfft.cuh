@@ -1,0 +1,358 @@
+// dm_warpfft.cuh -- warp-level register FFTs and the view-pipelined ("dataflow") psi update for
+// every frame edge N in {64, 128, 256, 512} (steps S1-S6 of DESIGN.md; eqs. (2)-(4) of
+// arXiv:1808.10375).  Included by dm_kernels.cuh.
+//
+// A frame of N >= 256 does not fit the registers / shared memory of one SM, so the 2-D FFT is
+// split at the row / column boundary and the intermediate spectra travel through a small ring
+// of scratch frames that stays resident in L2.  Every 1-D FFT is done by ONE WARP on 32 lanes x
+// 32 registers with a single in-warp 32 x 32 transpose (no block barrier):
+//
+//   line of length N = 32 RX (RX = N/32 in {2,4,8,16});  a warp holds G = 32/RX lines;
+//   register a = g RX + r of lane t holds element n = t + 32 r of line g
+//   stage 1   radix-RX over r (-> k1), twiddle w_N^(t k1)
+//   exchange  (lane t, reg a) -> (lane a, reg t)                        [dmreg::x1_write/x1_read]
+//   stage 2   radix-32 over t (-> k2):   frequency k = k1 + RX k2, held by lane a = g RX + k1
+//
+// Three phases per view, all running in ONE persistent kernel that pulls tasks from a queue in
+// an order in which every task only depends on tasks queued before it (so a resident CTA never
+// waits for a CTA that is not running):
+//   A (rows)    R = 2 P O - psi, forward FFT along x, spectrum rows -> scratch ("column-group"
+//               layout: group cg holds G adjacent kx as [y][c], 8 KiB contiguous)
+//   B (columns) for all M = K L modes of one column group: forward FFT along y, mode-summed
+//               modulus constraint (eq. (4)), inverse FFT along y, back to scratch in place
+//   C (rows)    inverse FFT along x, psi_new = psi_old + beta (G - P O)
+// Phase B of view v is queued D views after phase A of v, phase C another D views later; the
+// window of views in flight (psi + scratch) is a few tens of MB, so psi_old of phase C and both
+// scratch passes hit L2 and psi crosses HBM once in and once out.
+//
+// The FFT code is __host__ __device__: tests run it on the CPU through dm_host_fft2_path(path 4).
+#pragma once
+#include <cuda_runtime.h>
+
+#include "dm_fft.cuh"
+#include "dm_regfft.cuh"
+
+namespace dmwf {
+
+using namespace dmfft;
+
+constexpr int WF_NT = 256, WF_WARPS = 8;            // threads / warps per CTA
+constexpr int WF_XBUF = dmreg::X1_WARP;              // exchange bytes per warp (4608)
+
+// ---- 1-D FFT of G lines by one warp (emulated lane by lane on the host) -----------------
+// tw[k1 * 32 + t] = exp(-2 pi i t k1 / N)
+template <int RX> DM_HD void stage1_fwd(float2 (&u)[32], const float2 *tw, int t)
+{
+    constexpr int G = 32 / RX;
+#pragma unroll
+    for (int g = 0; g < G; ++g) {
+        float2 v[RX];
+#pragma unroll
+        for (int r = 0; r < RX; ++r) v[r] = u[g * RX + r];
+        Dft<RX, false>::run(v);
+        u[g * RX] = v[0];
+#pragma unroll
+        for (int k1 = 1; k1 < RX; ++k1) u[g * RX + k1] = cmul(v[k1], tw[k1 * 32 + t]);
+    }
+}
+
+template <int RX> DM_HD void stage1_inv(float2 (&u)[32], const float2 *tw, int t)
+{
+    constexpr int G = 32 / RX;
+#pragma unroll
+    for (int g = 0; g < G; ++g) {
+        float2 v[RX];
+        v[0] = u[g * RX];
+#pragma unroll
+        for (int k1 = 1; k1 < RX; ++k1) v[k1] = cmulc(u[g * RX + k1], tw[k1 * 32 + t]);
+        Dft<RX, true>::run(v);
+#pragma unroll
+        for (int r = 0; r < RX; ++r) u[g * RX + r] = v[r];
+    }
+}
+
+// ---- layouts ------------------------------------------------------------------------------
+// scratch frame: element (y, kx) at ((kx / G) N + y) G + kx % G        (G = 1024 / N columns per group)
+template <int N> DM_HD int scratch_index(int y, int kx)
+{
+    constexpr int G = 1024 / N;
+    return ((kx / G) * N + y) * G + kx % G;
+}
+// sqrt(I) storage: register k2 of lane a in column group cg sits at [cg][k2 >> 2][a][k2 & 3]
+DM_HD int spec_pos(int cg, int a, int k2) { return ((cg * 8 + (k2 >> 2)) * 32 + a) * 4 + (k2 & 3); }
+// natural-order frequency ky * N + kx held there after phase B's forward FFT
+template <int N> DM_HD int spec_freq(int cg, int a, int k2)
+{
+    constexpr int RX = N / 32, G = 32 / RX;
+    return ((a % RX) + RX * k2) * N + cg * G + a / RX;
+}
+
+} // namespace dmwf
+
+// =========================================================================================
+// The kernel (device only)
+// =========================================================================================
+#ifdef __CUDACC__
+
+namespace dmwf {
+
+struct WfArgs {
+    int n_views, K, L, H, W;
+    const int2 *pos;            // (y0, x0) per view
+    const float2 *P;            // [K][N][N]
+    const float2 *O;            // [L][H][W]
+    float2 *psi;                // [n_views][M][N][N], updated in place
+    const float *amp;           // [n_views][N*N] sqrt(I) in the layout of spec_pos
+    const float2 *tw;           // [RX][32]
+    float2 *scratch;            // [S][M][N*N] ring of spectrum frames
+    int S, D;                   // ring slots, phase lag in views
+    int nA, nB, nC;             // tasks per view and phase
+    int *queue;                 // task counter
+    int *cntA, *cntB, *cntC;    // [n_views] finished tasks per view and phase
+    float *partF;               // [n_views * nB][2]  (eF_num, eF_den)
+    float *partS;               // [n_views * nC][2]  (epsi_num, epsi_den)
+    float beta, eps;
+};
+
+__device__ __forceinline__ void spin_until(const int *cnt, int want)
+{
+    int v;
+    do {
+        asm volatile("ld.acquire.gpu.global.s32 %0, [%1];\n" : "=r"(v) : "l"(cnt) : "memory");
+        if (v < want) __nanosleep(64);
+    } while (v < want);
+}
+
+__device__ __forceinline__ float2 ldcg2(const float2 *p) { return __ldcg(p); }
+
+template <int N>
+__global__ void __launch_bounds__(WF_NT, 2) wf_dataflow_kernel(const WfArgs a)
+{
+    constexpr int RX = N / 32, G = 32 / RX, NN = N * N, NG = N / G;     // NG: column groups = row groups per frame
+    extern __shared__ __align__(16) unsigned char smem[];
+    unsigned char *xbuf = smem;                                           // [8 warps][WF_XBUF]
+    float4 *sumbuf = reinterpret_cast<float4 *>(smem + WF_WARPS * WF_XBUF);   // [8 warps][8][32] float4
+    float2 *s_tw = reinterpret_cast<float2 *>(smem + WF_WARPS * WF_XBUF + WF_WARPS * 4096);   // [RX][32]
+    __shared__ int s_task;
+    __shared__ float red[2 * WF_WARPS];
+
+    const int tid = threadIdx.x, w = tid >> 5, t = tid & 31;
+    const int M = a.K * a.L;
+    for (int i = tid; i < RX * 32; i += WF_NT) s_tw[i] = a.tw[i];
+    unsigned char *wbuf = xbuf + w * WF_XBUF;
+    const int T = a.nA + a.nB + a.nC;
+    const int total = (a.n_views + 2 * a.D) * T;
+    const int GPT = WF_WARPS / M;                                         // column groups per B task
+
+    for (;;) {
+        __syncthreads();
+        if (tid == 0) s_task = atomicAdd(a.queue, 1);
+        __syncthreads();
+        const int task = s_task;
+        if (task >= total) break;
+        const int step = task / T, rem = task % T;
+        int phase, sub, view;
+        if (rem < a.nA) { phase = 0; sub = rem; view = step; }
+        else if (rem < a.nA + a.nB) { phase = 1; sub = rem - a.nA; view = step - a.D; }
+        else { phase = 2; sub = rem - a.nA - a.nB; view = step - 2 * a.D; }
+        if (view < 0 || view >= a.n_views) continue;
+        // ---- dependencies (always on tasks queued earlier) ----
+        if (tid == 0) {
+            if (phase == 0) { if (view >= a.S) spin_until(a.cntC + view - a.S, a.nC); }
+            else if (phase == 1) spin_until(a.cntA + view, a.nA);
+            else spin_until(a.cntB + view, a.nB);
+        }
+        __syncthreads();
+        float2 *slot = a.scratch + (size_t)(view % a.S) * M * NN;
+        const int2 p0 = a.pos[view];
+        float2 u[32];
+        bool active;
+        float e0 = 0.f, e1 = 0.f;
+        // A / C geometry: row group rgi of the view -> frame m, rows y0 .. y0 + G - 1
+        const int rgi = sub * WF_WARPS + w;
+        const int m_ac = rgi / NG, y0 = (rgi % NG) * G;
+        // B geometry: warp -> (column group, mode)
+        const int cg = sub * GPT + w / M, m_b = w % M;
+        if (phase == 0) {
+            // ---- S1 + S2: R = 2 P O - psi, G rows of one mode frame ----
+            active = rgi < M * NG;
+            if (active) {
+                const int k = m_ac / a.L, l = m_ac % a.L;
+                const float2 *psi_f = a.psi + ((size_t)view * M + m_ac) * NN + (size_t)y0 * N + t;
+                const float2 *Pk = a.P + (size_t)k * NN + (size_t)y0 * N + t;
+                const float2 *Ow = a.O + (size_t)l * a.H * a.W + (size_t)(p0.x + y0) * a.W + p0.y + t;
+#pragma unroll
+                for (int i = 0; i < 32; ++i) u[i] = psi_f[(i / RX) * N + (i % RX) * 32];
+#pragma unroll
+                for (int g = 0; g < G; ++g) {
+                    float2 p[RX], o[RX];
+#pragma unroll
+                    for (int r = 0; r < RX; ++r) {
+                        p[r] = __ldg(Pk + g * N + r * 32);
+                        o[r] = __ldg(Ow + (size_t)g * a.W + r * 32);
+                    }
+#pragma unroll
+                    for (int r = 0; r < RX; ++r) {
+                        const float2 po = cmul(p[r], o[r]);
+                        u[g * RX + r] = make_float2(2.f * po.x - u[g * RX + r].x, 2.f * po.y - u[g * RX + r].y);
+                    }
+                }
+            }
+        } else if (phase == 1) {
+            // ---- spectrum rows of one column group, one mode: lane t holds y = t + 32 s ----
+            active = (w < GPT * M) && (cg < NG);
+            if (active) {
+                const float2 *src = slot + (size_t)m_b * NN + (size_t)cg * N * G + (size_t)t * G;
+#pragma unroll
+                for (int s = 0; s < RX; ++s)
+#pragma unroll
+                    for (int c = 0; c < G; c += 2) {
+                        const float4 v = __ldcg(reinterpret_cast<const float4 *>(src + (size_t)s * 32 * G + c));
+                        u[c * RX + s] = make_float2(v.x, v.y);
+                        u[(c + 1) * RX + s] = make_float2(v.z, v.w);
+                    }
+            }
+        } else {
+            // ---- scaled spectrum rows back from scratch: lane a = (g, k1), register k2 ----
+            active = rgi < M * NG;
+            if (active) {
+                const float2 *src = slot + (size_t)m_ac * NN;
+                const int g = t / RX, k1 = t % RX;
+#pragma unroll
+                for (int k2 = 0; k2 < 32; ++k2) u[k2] = ldcg2(src + scratch_index<N>(y0 + g, k1 + RX * k2));
+            }
+        }
+        // ---- forward FFT (A: along x, B: along y) ----
+        if (phase != 2 && active) {
+            stage1_fwd<RX>(u, s_tw, t);
+#pragma unroll
+            for (int rho = 0; rho < 2; ++rho) {
+                dmreg::x1_write(u, rho, t, wbuf);
+                __syncwarp();
+                dmreg::x1_read(u, rho, t, wbuf);
+                __syncwarp();
+            }
+            dmreg::dft32<false>(u);
+        }
+        // ---- S4: mode-summed modulus constraint (eq. (4)) ----
+        if (phase == 1) {
+            float4 *mine = sumbuf + (size_t)w * 256 + t;
+            if (active) {
+#pragma unroll
+                for (int j = 0; j < 8; ++j)
+                    mine[j * 32] = make_float4(dmreg::abs2_rn(u[4 * j]), dmreg::abs2_rn(u[4 * j + 1]),
+                                               dmreg::abs2_rn(u[4 * j + 2]), dmreg::abs2_rn(u[4 * j + 3]));
+            }
+            __syncthreads();
+            if (active) {
+                const float4 *ampv = reinterpret_cast<const float4 *>(a.amp + (size_t)view * NN) + (size_t)cg * 256 + t;
+                const float4 *peers = sumbuf + (size_t)(w - m_b) * 256 + t;
+                const float cfac = 1.f / (float)NN;
+#pragma unroll
+                for (int j = 0; j < 8; ++j) {
+                    const float4 am = __ldg(ampv + j * 32);
+                    float4 S = make_float4(0.f, 0.f, 0.f, 0.f);
+                    for (int mm = 0; mm < M; ++mm) {
+                        const float4 v = peers[(size_t)mm * 256 + j * 32];
+                        S.x += v.x; S.y += v.y; S.z += v.z; S.w += v.w;
+                    }
+                    const float Sv[4] = {S.x, S.y, S.z, S.w}, av[4] = {am.x, am.y, am.z, am.w};
+#pragma unroll
+                    for (int c = 0; c < 4; ++c) {
+                        const float rs = rsqrtf(Sv[c] + a.eps);
+                        const float d = Sv[c] * rs - av[c];
+                        e0 = fmaf(d, d, e0);
+                        e1 = fmaf(av[c], av[c], e1);
+                        const float sc = av[c] * rs * cfac;
+                        u[4 * j + c].x *= sc;
+                        u[4 * j + c].y *= sc;
+                    }
+                }
+                if (m_b != 0) { e0 = 0.f; e1 = 0.f; }
+            }
+        }
+        // ---- inverse FFT (B: along y, C: along x) ----
+        if (phase != 0 && active) {
+            dmreg::dft32<true>(u);
+#pragma unroll
+            for (int rho = 0; rho < 2; ++rho) {
+                dmreg::x1_write(u, rho, t, wbuf);
+                __syncwarp();
+                dmreg::x1_read(u, rho, t, wbuf);
+                __syncwarp();
+            }
+            stage1_inv<RX>(u, s_tw, t);
+        }
+        // ---- stores ----
+        if (phase == 0) {
+            if (active) {
+                float2 *dst = slot + (size_t)m_ac * NN;
+                const int g = t / RX, k1 = t % RX;
+#pragma unroll
+                for (int k2 = 0; k2 < 32; ++k2) __stcg(dst + scratch_index<N>(y0 + g, k1 + RX * k2), u[k2]);
+            }
+        } else if (phase == 1) {
+            if (active) {
+                float2 *dst = slot + (size_t)m_b * NN + (size_t)cg * N * G + (size_t)t * G;
+#pragma unroll
+                for (int s = 0; s < RX; ++s)
+#pragma unroll
+                    for (int c = 0; c < G; c += 2)
+                        __stcg(reinterpret_cast<float4 *>(dst + (size_t)s * 32 * G + c),
+                               make_float4(u[c * RX + s].x, u[c * RX + s].y, u[(c + 1) * RX + s].x, u[(c + 1) * RX + s].y));
+            }
+        } else {
+            // ---- S6: psi_new = psi_old + beta (G - P O) ----
+            if (active) {
+                const int k = m_ac / a.L, l = m_ac % a.L;
+                float2 *psi_f = a.psi + ((size_t)view * M + m_ac) * NN + (size_t)y0 * N + t;
+                const float2 *Pk = a.P + (size_t)k * NN + (size_t)y0 * N + t;
+                const float2 *Ow = a.O + (size_t)l * a.H * a.W + (size_t)(p0.x + y0) * a.W + p0.y + t;
+#pragma unroll
+                for (int g = 0; g < G; ++g) {
+                    float2 p[RX], o[RX], old[RX];
+#pragma unroll
+                    for (int r = 0; r < RX; ++r) {
+                        old[r] = __ldcs(psi_f + g * N + r * 32);
+                        p[r] = __ldg(Pk + g * N + r * 32);
+                        o[r] = __ldg(Ow + (size_t)g * a.W + r * 32);
+                    }
+#pragma unroll
+                    for (int r = 0; r < RX; ++r) {
+                        const float2 po = cmul(p[r], o[r]);
+                        const float tx = u[g * RX + r].x - po.x, ty = u[g * RX + r].y - po.y;
+                        const float2 nw = make_float2(fmaf(a.beta, tx, old[r].x), fmaf(a.beta, ty, old[r].y));
+                        e0 = fmaf(tx, tx, fmaf(ty, ty, e0));
+                        e1 = fmaf(nw.x, nw.x, fmaf(nw.y, nw.y, e1));
+                        __stcs(psi_f + g * N + r * 32, nw);
+                    }
+                }
+            }
+        }
+        // ---- publish: partial sums (fixed order) and the completion counter ----
+        if (phase != 0) {
+#pragma unroll
+            for (int s = 16; s > 0; s >>= 1) {
+                e0 += __shfl_xor_sync(0xffffffffu, e0, s);
+                e1 += __shfl_xor_sync(0xffffffffu, e1, s);
+            }
+            if (t == 0) { red[w] = e0; red[WF_WARPS + w] = e1; }
+        }
+        __threadfence();
+        __syncthreads();
+        if (tid == 0) {
+            if (phase != 0) {
+                float s0 = 0.f, s1 = 0.f;
+                for (int ww = 0; ww < WF_WARPS; ++ww) { s0 += red[ww]; s1 += red[WF_WARPS + ww]; }
+                float2 *out = reinterpret_cast<float2 *>(phase == 1 ? a.partF : a.partS) +
+                              ((size_t)view * (phase == 1 ? a.nB : a.nC) + sub);
+                *out = make_float2(phase == 2 ? s0 * a.beta * a.beta : s0, s1);
+            }
+            __threadfence();
+            atomicAdd((phase == 0 ? a.cntA : phase == 1 ? a.cntB : a.cntC) + view, 1);
+        }
+    }
+}
+
+} // namespace dmwf
+#endif // __CUDACC__

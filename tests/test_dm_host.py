@@ -153,3 +153,21 @@ def test_register_resident_fft_code_on_host(dm, rng):
     assert np.abs(dm.host_fft2(d, path=3) - want).max() < 1e-5
     with pytest.raises(dm.DMError):
         dm.host_fft2(np.zeros((64, 64), np.complex64), path=3)
+
+
+@pytest.mark.parametrize("N", [64, 128, 256, 512])
+def test_warp_fft_code_on_host(dm, N, rng):
+    """Path 4 (csrc/dm_warpfft.cuh): the warp-level stage-1 / exchange / stage-2 FFT, the
+    column-group scratch layout and the spectrum-layout table, emulated for one warp at a time
+    on the host (rows -> scratch -> columns), against the oracle FFT."""
+    x = (rng.standard_normal((N, N)) + 1j * rng.standard_normal((N, N))).astype(np.complex64)
+    F = dm.host_fft2(x, path=4)
+    Fo = oracle.fft2(x.astype(np.complex128))
+    assert synth.rel_l2(F, Fo) < 2e-6
+    xi = dm.host_fft2(Fo.astype(np.complex64), inverse=True, path=4)
+    assert synth.rel_l2(xi, x) < 2e-6
+    d = np.zeros((N, N), np.complex64)
+    d[7, 33] = 1
+    u = np.arange(N)
+    want = np.exp(-2j * np.pi * (7 * u[:, None] + 33 * u[None, :]) / N)
+    assert np.abs(dm.host_fft2(d, path=4) - want).max() < 1e-5

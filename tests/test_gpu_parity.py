@@ -64,12 +64,13 @@ def forced_pair(dm, pr, t_state, **params):
 
 
 @pytest.mark.parametrize("cfg_i,ny,nx", SMALL)
-@pytest.mark.parametrize("path", [0, 1, 2, 3])
+@pytest.mark.parametrize("path", [0, 1, 2, 3, 4])
 def test_one_iteration_parity(dm, cfg_i, ny, nx, path):
     """P2: set_data state (psi = P0*O0, frozen alphas) is exact; then one full iteration from an
     identical on-trajectory state (oracle state after 1 iteration) within 1e-5 on psi, P, O.
     path 0 = what dm_iterate picks (register-resident kernel for N = 128, fused shared-memory
-    kernel for N = 64, staged path above); 1, 2, 3 force the staged / fused / register path."""
+    kernel for N = 64, view-pipelined warp-FFT kernel above); 1, 2, 3, 4 force the staged /
+    fused / register-resident / warp-FFT path."""
     N = synth.CONFIGS[cfg_i].N
     if (path == 2 and N > 128) or (path == 3 and N != 128):
         pytest.skip("path not defined for this frame size")
