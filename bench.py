@@ -156,7 +156,7 @@ def run_ours(args, cfg):
     # every rank reconstructs its own data set (replicas; seed = rank)
     pr = synth.make_problem(cfg, seed=rank)
     plan = dm.DMPlan(cfg.N, cfg.n_views, cfg.K, cfg.L, cfg.obj_h, cfg.obj_w, pr.positions,
-                     path=args.path).alloc_workspace()
+                     path=args.path, **({"lag": args.lag} if args.lag else {})).alloc_workspace()
     I_h = torch.from_numpy(pr.intensities).pin_memory()
     P_h = torch.from_numpy(pr.probe0).pin_memory()
     O_h = torch.from_numpy(pr.object0).pin_memory()
@@ -264,6 +264,7 @@ def main():
     ap.add_argument("--config", type=int, default=1, help="BASELINE.json config index (default 1)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--path", type=int, default=0, help="0 auto, 1 staged, 2 fused")
+    ap.add_argument("--lag", type=int, default=0, help="path 4: phase lag in views (0 = derived)")
     ap.add_argument("--e2e-steps", type=int, default=20)
     ap.add_argument("--ref-mode-views", type=int, default=4096,
                     help="size of the bounded oracle sample (mode-views per iteration)")

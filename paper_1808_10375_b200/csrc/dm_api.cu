@@ -38,7 +38,7 @@ struct dm_plan {
     int path_req, path;                  // requested / chosen (1 staged, 2 fused, 3 register-resident)
     int reg_grid;                        // path 3: number of persistent CTAs (multiple of M)
     // path 4 (dm_warpfft.cuh): ring slots, phase lag (views), tasks per view and phase, persistent CTAs
-    int wf_S, wf_D, wf_nA, wf_nB, wf_nC, wf_grid;
+    int wf_S, wf_D, wf_nA, wf_nB, wf_nC, wf_grid, wf_nw;
     int wf_lag_req;                      // 0 = derive the lag from the task counts
     int *wf_cnt;                         // [1 + 3 n_views] queue counter, cntA, cntB, cntC
     float2 *wf_tw_d;                     // [N/32][32] stage-1 twiddles
@@ -145,13 +145,17 @@ void plan_geometry(dm_plan *p)
     if (cv > (size_t)p->n_views) cv = p->n_views;
     p->chunk_views = (int)cv;
     // path 4: a CTA task = 8 row groups (phases A, C) or 8 / M column groups x M modes (phase B)
-    const int G = 1024 / p->N, NG = p->N / G, GPT = dmwf::WF_WARPS / p->M;
-    p->wf_nA = (p->M * NG + dmwf::WF_WARPS - 1) / dmwf::WF_WARPS;
+    const int G = 1024 / p->N, NG = p->N / G;
+    p->wf_nw = p->M == 1 ? 2 : p->M;                 // warps per CTA
+    const int GPT = p->wf_nw / p->M;
+    p->wf_nA = (p->M * NG + p->wf_nw - 1) / p->wf_nw;
     p->wf_nC = p->wf_nA;
     p->wf_nB = (NG + GPT - 1) / GPT;
     const int T = p->wf_nA + p->wf_nB + p->wf_nC;
-    // lag: a phase starts on a view once ~1.2 x (resident CTAs = 2 x 148) tasks have been queued behind its inputs
-    int D = p->wf_lag_req > 0 ? p->wf_lag_req : (int)((1.2 * 296 + T - 1) / T);
+    // lag: a phase starts on a view once ~2.4 x (resident CTAs) tasks have been queued behind its inputs
+    // (measured on B200: c3 lag 4 and c1 lag 60 beat half those lags by 10 %; psi + ring still fit L2)
+    const int resident = 148 * (16 / p->wf_nw);
+    int D = p->wf_lag_req > 0 ? p->wf_lag_req : (int)((2.4 * resident + T - 1) / T);
     if (D < 1) D = 1;
     p->wf_D = D;
     p->wf_S = 2 * D + 4;
@@ -339,17 +343,19 @@ dm_status launch_regfft(dm_plan *plan, cudaStream_t st, bool query_only)
 template <int N> dm_status launch_wf_t(dm_plan *plan, cudaStream_t st, bool query_only)
 {
     auto kern = dmwf::wf_dataflow_kernel<N>;
-    const int smem = dmwf::WF_WARPS * dmwf::WF_XBUF + dmwf::WF_WARPS * 4096 + (N / 32) * 32 * (int)sizeof(float2);
+    const int nt = 32 * plan->wf_nw;
+    const int smem = plan->wf_nw * dmwf::WF_XBUF + (N / 32) * 32 * (int)sizeof(float2);
     static bool attr_done = false;
     if (!attr_done) {
-        CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+        CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                dmwf::WF_MAXW * dmwf::WF_XBUF + (N / 32) * 32 * (int)sizeof(float2)));
         attr_done = true;
     }
     if (query_only) {
         int dev = 0, sms = 0, per = 0;
         CU(cudaGetDevice(&dev));
         CU(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
-        CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per, kern, dmwf::WF_NT, smem));
+        CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per, kern, nt, smem));
         if (per < 1) return fail(plan, DM_ERR_CUDA, "warp-FFT kernel does not fit an SM");
         plan->wf_grid = sms * per;
         return DM_OK;
@@ -366,7 +372,7 @@ template <int N> dm_status launch_wf_t(dm_plan *plan, cudaStream_t st, bool quer
     CU(cudaMemsetAsync(plan->wf_cnt, 0, (1 + 3 * (size_t)plan->n_views) * sizeof(int), st));
     const long long tasks = (long long)(plan->n_views + 2 * plan->wf_D) * (plan->wf_nA + plan->wf_nB + plan->wf_nC);
     const int grid = tasks < plan->wf_grid ? (int)tasks : plan->wf_grid;
-    kern<<<grid, dmwf::WF_NT, smem, st>>>(a);
+    kern<<<grid, nt, smem, st>>>(a);
     CU(cudaGetLastError());
     return DM_OK;
 }
@@ -958,10 +964,8 @@ template <int N> void host_fft2_wf(const float *in, float *out, int inverse)
         }
     auto U = [&](int lane) -> float2(&)[32] { return *reinterpret_cast<float2(*)[32]>(&regs[(size_t)lane * 32]); };
     auto exch = [&]() {
-        for (int rho = 0; rho < 2; ++rho) {
-            for (int t = 0; t < 32; ++t) dmreg::x1_write(U(t), rho, t, xbuf);
-            for (int t = 0; t < 32; ++t) dmreg::x1_read(U(t), rho, t, xbuf);
-        }
+        for (int t = 0; t < 32; ++t) xt_write(U(t), t, xbuf);
+        for (int t = 0; t < 32; ++t) xt_read(U(t), t, xbuf);
     };
     auto fwd = [&]() {
         for (int t = 0; t < 32; ++t) stage1_fwd<RX>(U(t), tw.data(), t);

@@ -36,8 +36,28 @@ namespace dmwf {
 
 using namespace dmfft;
 
-constexpr int WF_NT = 256, WF_WARPS = 8;            // threads / warps per CTA
-constexpr int WF_XBUF = dmreg::X1_WARP;              // exchange bytes per warp (4608)
+constexpr int WF_MAXW = 8;                           // warps per CTA: M = K L (2 if M = 1)
+constexpr int WF_ROW = 272, WF_XBUF = 32 * WF_ROW;   // exchange buffer of one warp: 32 rows of 32 c64 + 16 B pad
+
+// ---- in-warp 32 x 32 transpose (lane t, reg a) -> (lane a, reg t), one round -------------
+// Every lane writes its 32 registers down a column (64-bit stores: the 16 lanes of a half warp
+// fill 128 contiguous bytes) and reads one padded row back (128-bit loads, row stride 272 B:
+// the 8 lanes of a quarter warp hit 8 different 16-byte bank groups).  No lane-dependent
+// register choice, so no divergence.  wbuf = this warp's WF_XBUF bytes.
+DM_HD void xt_write(const float2 (&u)[32], int t, unsigned char *wbuf)
+{
+#pragma unroll
+    for (int a = 0; a < 32; ++a) *reinterpret_cast<float2 *>(wbuf + a * WF_ROW + t * 8) = u[a];
+}
+DM_HD void xt_read(float2 (&u)[32], int t, const unsigned char *wbuf)
+{
+#pragma unroll
+    for (int b = 0; b < 32; b += 2) {
+        const float4 v = *reinterpret_cast<const float4 *>(wbuf + t * WF_ROW + b * 8);
+        u[b] = make_float2(v.x, v.y);
+        u[b + 1] = make_float2(v.z, v.w);
+    }
+}
 
 // ---- 1-D FFT of G lines by one warp (emulated lane by lane on the host) -----------------
 // tw[k1 * 32 + t] = exp(-2 pi i t k1 / N)
@@ -117,62 +137,99 @@ struct WfArgs {
 __device__ __forceinline__ void spin_until(const int *cnt, int want)
 {
     int v;
-    do {
+    for (;;) {
         asm volatile("ld.acquire.gpu.global.s32 %0, [%1];\n" : "=r"(v) : "l"(cnt) : "memory");
-        if (v < want) __nanosleep(64);
-    } while (v < want);
+        if (v >= want) break;
+        __nanosleep(100);
+    }
 }
 
-__device__ __forceinline__ float2 ldcg2(const float2 *p) { return __ldcg(p); }
+__device__ __forceinline__ float abs2_rn(float2 f) { return __fmaf_rn(f.y, f.y, __fmul_rn(f.x, f.x)); }
 
+// forward / inverse 1-D FFT of the warp's G lines (registers <-> registers)
+template <int RX> __device__ __forceinline__ void warp_fft_fwd(float2 (&u)[32], const float2 *s_tw, int t, unsigned char *wbuf)
+{
+    stage1_fwd<RX>(u, s_tw, t);
+    xt_write(u, t, wbuf);
+    __syncwarp();
+    xt_read(u, t, wbuf);
+    __syncwarp();
+    dmreg::dft32<false>(u);
+}
+template <int RX> __device__ __forceinline__ void warp_fft_inv(float2 (&u)[32], const float2 *s_tw, int t, unsigned char *wbuf)
+{
+    dmreg::dft32<true>(u);
+    xt_write(u, t, wbuf);
+    __syncwarp();
+    xt_read(u, t, wbuf);
+    __syncwarp();
+    stage1_inv<RX>(u, s_tw, t);
+}
+
+// One CTA = NW = blockDim.x / 32 warps (a multiple of M).  A task is NW row groups of a view
+// (phases A, C) or NW / M column groups x M modes (phase B).
 template <int N>
-__global__ void __launch_bounds__(WF_NT, 2) wf_dataflow_kernel(const WfArgs a)
+__global__ void __launch_bounds__(32 * WF_MAXW, 2) wf_dataflow_kernel(const WfArgs a)
 {
     constexpr int RX = N / 32, G = 32 / RX, NN = N * N, NG = N / G;     // NG: column groups = row groups per frame
     extern __shared__ __align__(16) unsigned char smem[];
-    unsigned char *xbuf = smem;                                           // [8 warps][WF_XBUF]
-    float4 *sumbuf = reinterpret_cast<float4 *>(smem + WF_WARPS * WF_XBUF);   // [8 warps][8][32] float4
-    float2 *s_tw = reinterpret_cast<float2 *>(smem + WF_WARPS * WF_XBUF + WF_WARPS * 4096);   // [RX][32]
-    __shared__ int s_task;
-    __shared__ float red[2 * WF_WARPS];
+    __shared__ int s_task[2];
+    __shared__ float red[2 * WF_MAXW];
 
-    const int tid = threadIdx.x, w = tid >> 5, t = tid & 31;
+    const int tid = threadIdx.x, w = tid >> 5, t = tid & 31, NW = blockDim.x >> 5;
     const int M = a.K * a.L;
-    for (int i = tid; i < RX * 32; i += WF_NT) s_tw[i] = a.tw[i];
-    unsigned char *wbuf = xbuf + w * WF_XBUF;
+    unsigned char *wbuf = smem + w * WF_XBUF;                 // exchange buffer; doubles as the |F|^2 buffer
+    float2 *s_tw = reinterpret_cast<float2 *>(smem + NW * WF_XBUF);       // [RX][32]
+    for (int i = tid; i < RX * 32; i += blockDim.x) s_tw[i] = a.tw[i];
     const int T = a.nA + a.nB + a.nC;
     const int total = (a.n_views + 2 * a.D) * T;
-    const int GPT = WF_WARPS / M;                                         // column groups per B task
+    const int GPT = NW / M;                                               // column groups per B task
 
-    for (;;) {
-        __syncthreads();
-        if (tid == 0) s_task = atomicAdd(a.queue, 1);
-        __syncthreads();
-        const int task = s_task;
-        if (task >= total) break;
-        const int step = task / T, rem = task % T;
-        int phase, sub, view;
+    // task -> (phase, sub, view); view outside [0, n_views) = nothing to do
+    auto decode = [&](int task, int &phase, int &sub, int &view) {
+        const int step = task / T, rem = task - step * T;
         if (rem < a.nA) { phase = 0; sub = rem; view = step; }
         else if (rem < a.nA + a.nB) { phase = 1; sub = rem - a.nA; view = step - a.D; }
         else { phase = 2; sub = rem - a.nA - a.nB; view = step - 2 * a.D; }
-        if (view < 0 || view >= a.n_views) continue;
-        // ---- dependencies (always on tasks queued earlier) ----
-        if (tid == 0) {
-            if (phase == 0) { if (view >= a.S) spin_until(a.cntC + view - a.S, a.nC); }
-            else if (phase == 1) spin_until(a.cntA + view, a.nA);
-            else spin_until(a.cntB + view, a.nB);
+    };
+    // thread 0: claim the next task that has work and wait for what it depends on (always tasks
+    // queued earlier, hence finished or running on a resident CTA)
+    auto resolve = [&](int task) -> int {
+        for (;;) {
+            if (task >= total) return task;
+            int phase, sub, view;
+            decode(task, phase, sub, view);
+            if (view >= 0 && view < a.n_views) {
+                if (phase == 0) { if (view >= a.S) spin_until(a.cntC + view - a.S, a.nC); }
+                else if (phase == 1) spin_until(a.cntA + view, a.nA);
+                else spin_until(a.cntB + view, a.nB);
+                return task;
+            }
+            task = atomicAdd(a.queue, 1);
         }
-        __syncthreads();
+    };
+    if (tid == 0) s_task[0] = resolve(atomicAdd(a.queue, 1));
+    __syncthreads();
+
+    for (int buf = 0;; buf ^= 1) {
+        const int task = s_task[buf];
+        if (task >= total) break;
+        int nxt = 0;
+        if (tid == 0) nxt = atomicAdd(a.queue, 1);            // in flight while this task runs
+        int phase, sub, view;
+        decode(task, phase, sub, view);
         float2 *slot = a.scratch + (size_t)(view % a.S) * M * NN;
         const int2 p0 = a.pos[view];
         float2 u[32];
         bool active;
         float e0 = 0.f, e1 = 0.f;
         // A / C geometry: row group rgi of the view -> frame m, rows y0 .. y0 + G - 1
-        const int rgi = sub * WF_WARPS + w;
+        const int rgi = sub * NW + w;
         const int m_ac = rgi / NG, y0 = (rgi % NG) * G;
         // B geometry: warp -> (column group, mode)
         const int cg = sub * GPT + w / M, m_b = w % M;
+        // scratch address of (row y0 + t / RX, kx = t % RX) -- register k2 adds scratch_index(0, RX k2)
+        const int sidx = scratch_index<N>(y0 + t / RX, t % RX);
         if (phase == 0) {
             // ---- S1 + S2: R = 2 P O - psi, G rows of one mode frame ----
             active = rgi < M * NG;
@@ -184,17 +241,18 @@ __global__ void __launch_bounds__(WF_NT, 2) wf_dataflow_kernel(const WfArgs a)
 #pragma unroll
                 for (int i = 0; i < 32; ++i) u[i] = psi_f[(i / RX) * N + (i % RX) * 32];
 #pragma unroll
-                for (int g = 0; g < G; ++g) {
-                    float2 p[RX], o[RX];
+                for (int h = 0; h < 2; ++h) {
+                    float2 p[16], o[16];
 #pragma unroll
-                    for (int r = 0; r < RX; ++r) {
-                        p[r] = __ldg(Pk + g * N + r * 32);
-                        o[r] = __ldg(Ow + (size_t)g * a.W + r * 32);
+                    for (int i = 0; i < 16; ++i) {
+                        const int e = 16 * h + i;
+                        p[i] = __ldg(Pk + (e / RX) * N + (e % RX) * 32);
+                        o[i] = __ldg(Ow + (size_t)(e / RX) * a.W + (e % RX) * 32);
                     }
 #pragma unroll
-                    for (int r = 0; r < RX; ++r) {
-                        const float2 po = cmul(p[r], o[r]);
-                        u[g * RX + r] = make_float2(2.f * po.x - u[g * RX + r].x, 2.f * po.y - u[g * RX + r].y);
+                    for (int i = 0; i < 16; ++i) {
+                        const float2 po = cmul(p[i], o[i]);
+                        u[16 * h + i] = make_float2(2.f * po.x - u[16 * h + i].x, 2.f * po.y - u[16 * h + i].y);
                     }
                 }
             }
@@ -216,46 +274,36 @@ __global__ void __launch_bounds__(WF_NT, 2) wf_dataflow_kernel(const WfArgs a)
             // ---- scaled spectrum rows back from scratch: lane a = (g, k1), register k2 ----
             active = rgi < M * NG;
             if (active) {
-                const float2 *src = slot + (size_t)m_ac * NN;
-                const int g = t / RX, k1 = t % RX;
+                const float2 *src = slot + (size_t)m_ac * NN + sidx;
 #pragma unroll
-                for (int k2 = 0; k2 < 32; ++k2) u[k2] = ldcg2(src + scratch_index<N>(y0 + g, k1 + RX * k2));
+                for (int k2 = 0; k2 < 32; ++k2) u[k2] = __ldcg(src + scratch_index<N>(0, RX * k2));
             }
         }
         // ---- forward FFT (A: along x, B: along y) ----
-        if (phase != 2 && active) {
-            stage1_fwd<RX>(u, s_tw, t);
-#pragma unroll
-            for (int rho = 0; rho < 2; ++rho) {
-                dmreg::x1_write(u, rho, t, wbuf);
-                __syncwarp();
-                dmreg::x1_read(u, rho, t, wbuf);
-                __syncwarp();
-            }
-            dmreg::dft32<false>(u);
-        }
+        if (phase != 2 && active) warp_fft_fwd<RX>(u, s_tw, t, wbuf);
         // ---- S4: mode-summed modulus constraint (eq. (4)) ----
         if (phase == 1) {
-            float4 *mine = sumbuf + (size_t)w * 256 + t;
+            float4 *mine = reinterpret_cast<float4 *>(wbuf) + t;
             if (active) {
 #pragma unroll
                 for (int j = 0; j < 8; ++j)
-                    mine[j * 32] = make_float4(dmreg::abs2_rn(u[4 * j]), dmreg::abs2_rn(u[4 * j + 1]),
-                                               dmreg::abs2_rn(u[4 * j + 2]), dmreg::abs2_rn(u[4 * j + 3]));
+                    mine[j * 32] = make_float4(abs2_rn(u[4 * j]), abs2_rn(u[4 * j + 1]), abs2_rn(u[4 * j + 2]), abs2_rn(u[4 * j + 3]));
             }
             __syncthreads();
             if (active) {
                 const float4 *ampv = reinterpret_cast<const float4 *>(a.amp + (size_t)view * NN) + (size_t)cg * 256 + t;
-                const float4 *peers = sumbuf + (size_t)(w - m_b) * 256 + t;
+                const unsigned char *peers = smem + (size_t)(w - m_b) * WF_XBUF;
                 const float cfac = 1.f / (float)NN;
 #pragma unroll
                 for (int j = 0; j < 8; ++j) {
                     const float4 am = __ldg(ampv + j * 32);
                     float4 S = make_float4(0.f, 0.f, 0.f, 0.f);
-                    for (int mm = 0; mm < M; ++mm) {
-                        const float4 v = peers[(size_t)mm * 256 + j * 32];
-                        S.x += v.x; S.y += v.y; S.z += v.z; S.w += v.w;
-                    }
+#pragma unroll
+                    for (int mm = 0; mm < WF_MAXW; ++mm)
+                        if (mm < M) {
+                            const float4 v = reinterpret_cast<const float4 *>(peers + (size_t)mm * WF_XBUF)[j * 32 + t];
+                            S.x += v.x; S.y += v.y; S.z += v.z; S.w += v.w;
+                        }
                     const float Sv[4] = {S.x, S.y, S.z, S.w}, av[4] = {am.x, am.y, am.z, am.w};
 #pragma unroll
                     for (int c = 0; c < 4; ++c) {
@@ -270,26 +318,16 @@ __global__ void __launch_bounds__(WF_NT, 2) wf_dataflow_kernel(const WfArgs a)
                 }
                 if (m_b != 0) { e0 = 0.f; e1 = 0.f; }
             }
+            __syncthreads();            // every warp has read the |F|^2 buffers before they serve as exchange buffers again
         }
         // ---- inverse FFT (B: along y, C: along x) ----
-        if (phase != 0 && active) {
-            dmreg::dft32<true>(u);
-#pragma unroll
-            for (int rho = 0; rho < 2; ++rho) {
-                dmreg::x1_write(u, rho, t, wbuf);
-                __syncwarp();
-                dmreg::x1_read(u, rho, t, wbuf);
-                __syncwarp();
-            }
-            stage1_inv<RX>(u, s_tw, t);
-        }
+        if (phase != 0 && active) warp_fft_inv<RX>(u, s_tw, t, wbuf);
         // ---- stores ----
         if (phase == 0) {
             if (active) {
-                float2 *dst = slot + (size_t)m_ac * NN;
-                const int g = t / RX, k1 = t % RX;
+                float2 *dst = slot + (size_t)m_ac * NN + sidx;
 #pragma unroll
-                for (int k2 = 0; k2 < 32; ++k2) __stcg(dst + scratch_index<N>(y0 + g, k1 + RX * k2), u[k2]);
+                for (int k2 = 0; k2 < 32; ++k2) __stcg(dst + scratch_index<N>(0, RX * k2), u[k2]);
             }
         } else if (phase == 1) {
             if (active) {
@@ -309,48 +347,51 @@ __global__ void __launch_bounds__(WF_NT, 2) wf_dataflow_kernel(const WfArgs a)
                 const float2 *Pk = a.P + (size_t)k * NN + (size_t)y0 * N + t;
                 const float2 *Ow = a.O + (size_t)l * a.H * a.W + (size_t)(p0.x + y0) * a.W + p0.y + t;
 #pragma unroll
-                for (int g = 0; g < G; ++g) {
-                    float2 p[RX], o[RX], old[RX];
+                for (int h = 0; h < 4; ++h) {
+                    float2 p[8], o[8], old[8];
 #pragma unroll
-                    for (int r = 0; r < RX; ++r) {
-                        old[r] = __ldcs(psi_f + g * N + r * 32);
-                        p[r] = __ldg(Pk + g * N + r * 32);
-                        o[r] = __ldg(Ow + (size_t)g * a.W + r * 32);
+                    for (int i = 0; i < 8; ++i) {
+                        const int e = 8 * h + i;
+                        old[i] = __ldcs(psi_f + (e / RX) * N + (e % RX) * 32);
+                        p[i] = __ldg(Pk + (e / RX) * N + (e % RX) * 32);
+                        o[i] = __ldg(Ow + (size_t)(e / RX) * a.W + (e % RX) * 32);
                     }
 #pragma unroll
-                    for (int r = 0; r < RX; ++r) {
-                        const float2 po = cmul(p[r], o[r]);
-                        const float tx = u[g * RX + r].x - po.x, ty = u[g * RX + r].y - po.y;
-                        const float2 nw = make_float2(fmaf(a.beta, tx, old[r].x), fmaf(a.beta, ty, old[r].y));
+                    for (int i = 0; i < 8; ++i) {
+                        const int e = 8 * h + i;
+                        const float2 po = cmul(p[i], o[i]);
+                        const float tx = u[e].x - po.x, ty = u[e].y - po.y;
+                        const float2 nw = make_float2(fmaf(a.beta, tx, old[i].x), fmaf(a.beta, ty, old[i].y));
                         e0 = fmaf(tx, tx, fmaf(ty, ty, e0));
                         e1 = fmaf(nw.x, nw.x, fmaf(nw.y, nw.y, e1));
-                        __stcs(psi_f + g * N + r * 32, nw);
+                        __stcs(psi_f + (e / RX) * N + (e % RX) * 32, nw);
                     }
                 }
             }
         }
-        // ---- publish: partial sums (fixed order) and the completion counter ----
+        // ---- publish: partial sums (fixed order), completion counter, next task ----
         if (phase != 0) {
 #pragma unroll
             for (int s = 16; s > 0; s >>= 1) {
                 e0 += __shfl_xor_sync(0xffffffffu, e0, s);
                 e1 += __shfl_xor_sync(0xffffffffu, e1, s);
             }
-            if (t == 0) { red[w] = e0; red[WF_WARPS + w] = e1; }
+            if (t == 0) { red[w] = e0; red[WF_MAXW + w] = e1; }
         }
-        __threadfence();
         __syncthreads();
         if (tid == 0) {
             if (phase != 0) {
                 float s0 = 0.f, s1 = 0.f;
-                for (int ww = 0; ww < WF_WARPS; ++ww) { s0 += red[ww]; s1 += red[WF_WARPS + ww]; }
+                for (int ww = 0; ww < NW; ++ww) { s0 += red[ww]; s1 += red[WF_MAXW + ww]; }
                 float2 *out = reinterpret_cast<float2 *>(phase == 1 ? a.partF : a.partS) +
                               ((size_t)view * (phase == 1 ? a.nB : a.nC) + sub);
                 *out = make_float2(phase == 2 ? s0 * a.beta * a.beta : s0, s1);
             }
             __threadfence();
             atomicAdd((phase == 0 ? a.cntA : phase == 1 ? a.cntB : a.cntC) + view, 1);
+            s_task[buf ^ 1] = resolve(nxt);
         }
+        __syncthreads();
     }
 }
 
