@@ -249,7 +249,14 @@ struct RegArgs {
     float beta, eps;
 };
 
-constexpr int REG_SMEM_V1 = XBUF_BYTES + 2048;               // exchange buffer + twiddles
+// shared memory: [prefetch buffer 128 KiB | exchange buffer | twiddles 2 KiB]
+// The prefetch buffer is filled by bulk asynchronous copies (TMA, cp.async.bulk) one step ahead:
+//   half A (64 KiB): rows 0..63 of the next frame's psi, then -- once S1 has consumed them --
+//                    sqrt(I) of the current view (consumed by S4), then the next psi rows again
+//   half B (64 KiB): rows 64..127 of the next frame's psi
+// so the HBM time of a frame hides behind the FFTs of the previous / current frame.
+constexpr int PBUF_BYTES = 2 * 65536;
+constexpr int REG_SMEM_V1 = PBUF_BYTES + XBUF_BYTES + 2048;
 
 __device__ __forceinline__ float abs2_rn(float2 f) { return __fmaf_rn(f.y, f.y, __fmul_rn(f.x, f.x)); }
 
@@ -277,6 +284,31 @@ __device__ __forceinline__ void tmem_ld8(uint32_t taddr, float2 &a, float2 &b, f
 }
 __device__ __forceinline__ void tmem_wait_st() { asm volatile("tcgen05.wait::st.sync.aligned;\n" ::: "memory"); }
 __device__ __forceinline__ void tmem_wait_ld() { asm volatile("tcgen05.wait::ld.sync.aligned;\n" ::: "memory"); }
+// ---- mbarrier + 1-D bulk copy (global -> this CTA's shared memory) ----------------------------
+__device__ __forceinline__ void mbar_init(uint64_t *bar, uint32_t count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;\n" :: "r"((uint32_t)__cvta_generic_to_shared(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity)
+{
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "WAIT_%=:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra DONE_%=;\n"
+        "bra WAIT_%=;\n"
+        "DONE_%=:\n"
+        "}\n" :: "r"((uint32_t)__cvta_generic_to_shared(bar)), "r"(parity) : "memory");
+}
+// one thread: announce `bytes` on the barrier and start the copy that will deliver them
+__device__ __forceinline__ void bulk_load(void *dst_smem, const void *src_gmem, uint32_t bytes, uint64_t *bar)
+{
+    const uint32_t b = (uint32_t)__cvta_generic_to_shared(bar), d = (uint32_t)__cvta_generic_to_shared(dst_smem);
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;\n" :: "r"(b), "r"(bytes) : "memory");
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];\n"
+                 :: "r"(d), "l"(src_gmem), "r"(bytes), "r"(b) : "memory");
+}
 __device__ __forceinline__ void cluster_arrive() { asm volatile("barrier.cluster.arrive.release.aligned;\n" ::: "memory"); }
 __device__ __forceinline__ void cluster_wait() { asm volatile("barrier.cluster.wait.acquire.aligned;\n" ::: "memory"); }
 
@@ -287,11 +319,13 @@ __global__ void __launch_bounds__(RNT, 1) regfft128_kernel(const RegArgs a)
 {
     namespace cg = cooperative_groups;
     extern __shared__ __align__(16) unsigned char smem[];
-    unsigned char *xbuf = smem;
-    float2 *s_wy = reinterpret_cast<float2 *>(smem + XBUF_BYTES);
+    unsigned char *pbuf = smem;
+    unsigned char *xbuf = smem + PBUF_BYTES;
+    float2 *s_wy = reinterpret_cast<float2 *>(smem + PBUF_BYTES + XBUF_BYTES);
     float2 *s_wx = s_wy + 128;
     __shared__ float red[4 * 32];
     __shared__ uint32_t s_tmem;
+    __shared__ __align__(8) uint64_t mb_lo, mb_hi, mb_amp;      // psi rows 0..63 (half A), rows 64..127 (half B), sqrt(I) (half A)
 
     const int tid = threadIdx.x, w = tid >> 5, t = tid & 31;
     const int M = MT ? MT : a.K * a.L;
@@ -299,6 +333,12 @@ __global__ void __launch_bounds__(RNT, 1) regfft128_kernel(const RegArgs a)
     const int k = m / a.L, l = m % a.L;
     if (tid < 128) s_wy[tid] = a.wy[tid];
     else if (tid < 256) s_wx[tid - 128] = a.wx[tid - 128];
+    if (tid == 0) {
+        mbar_init(&mb_lo, 1);
+        mbar_init(&mb_hi, 1);
+        mbar_init(&mb_amp, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
+    }
     if (w == 0) {       // all 512 TMEM columns (this kernel is the only resident CTA of its SM)
         asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;\n"
                      :: "r"((uint32_t)__cvta_generic_to_shared(&s_tmem)), "r"(512) : "memory");
@@ -317,31 +357,57 @@ __global__ void __launch_bounds__(RNT, 1) regfft128_kernel(const RegArgs a)
     const float cfac = a.beta > 0.f ? 1.f / (float)RNN : 0.f;
     float e0 = 0.f, e1 = 0.f, e2 = 0.f, e3 = 0.f;
     int par = 0;
+    if (tid == 0 && cl < a.n_views) {       // first frame: both halves now
+        const unsigned char *src = reinterpret_cast<const unsigned char *>(a.psi + ((size_t)cl * M + m) * RNN);
+        bulk_load(pbuf, src, 65536, &mb_lo);
+        bulk_load(pbuf + 65536, src + 65536, 65536, &mb_hi);
+    }
 
     for (int view = cl; view < a.n_views; view += ncl, par ^= 1) {
         const int2 p0 = a.pos[view];
         float2 *psi_f = a.psi + ((size_t)view * M + m) * RNN + w * RN + t;
         const float2 *Ow = a.O + (size_t)l * a.H * a.W + (size_t)(p0.x + w) * a.W + p0.y + t;
+        const int nview = view + ncl;
+        const unsigned char *nsrc = reinterpret_cast<const unsigned char *>(a.psi + ((size_t)nview * M + m) * RNN);
         float2 u[32];
         // ---- S1 + S2: R = 2 P O - psi in L0; psi_old and P*O parked in tensor memory ----
+        // P and O come from L2: all of P and half of O are requested before anything else (psi still
+        // sits in shared memory, so the registers are free), the other half of O while the first is used.
+        {
+            float2 po[32], o[16];
 #pragma unroll
-        for (int r = 0; r < 32; ++r) u[r] = psi_f[(r >> 2) * 16 * RN + (r & 3) * 32];
+            for (int e = 0; e < 32; ++e) po[e] = __ldg(Pk + (e >> 2) * 16 * RN + (e & 3) * 32);
 #pragma unroll
-        for (int i = 0; i < 8; ++i) {
-            float2 p[4], o[4];
+            for (int e = 0; e < 16; ++e) o[e] = __ldg(Ow + (size_t)(e >> 2) * 16 * a.W + (e & 3) * 32);
+            mbar_wait(&mb_lo, par);
+            mbar_wait(&mb_hi, par);
+            const float2 *ps = reinterpret_cast<const float2 *>(pbuf) + w * RN + t;
 #pragma unroll
-            for (int r = 0; r < 4; ++r) {
-                p[r] = __ldg(Pk + i * 16 * RN + r * 32);
-                o[r] = __ldg(Ow + (size_t)i * 16 * a.W + r * 32);
+            for (int e = 0; e < 16; ++e) po[e] = cmul(po[e], o[e]);
+#pragma unroll
+            for (int e = 0; e < 16; ++e) o[e] = __ldg(Ow + (size_t)((e + 16) >> 2) * 16 * a.W + (e & 3) * 32);
+#pragma unroll
+            for (int h = 0; h < 2; ++h) {
+                if (h == 1) {
+#pragma unroll
+                    for (int e = 0; e < 16; ++e) po[16 + e] = cmul(po[16 + e], o[e]);
+                }
+#pragma unroll
+                for (int i = 4 * h; i < 4 * h + 4; ++i) {
+#pragma unroll
+                    for (int r = 0; r < 4; ++r) u[4 * i + r] = ps[i * 16 * RN + r * 32];
+                    tmem_st8(t_psi + 8 * i, u[4 * i], u[4 * i + 1], u[4 * i + 2], u[4 * i + 3]);
+                    tmem_st8(t_po + 8 * i, po[4 * i], po[4 * i + 1], po[4 * i + 2], po[4 * i + 3]);
+#pragma unroll
+                    for (int r = 0; r < 4; ++r)
+                        u[4 * i + r] = make_float2(2.f * po[4 * i + r].x - u[4 * i + r].x, 2.f * po[4 * i + r].y - u[4 * i + r].y);
+                }
             }
-            tmem_st8(t_psi + 8 * i, u[4 * i], u[4 * i + 1], u[4 * i + 2], u[4 * i + 3]);
-            float2 po[4];
-#pragma unroll
-            for (int r = 0; r < 4; ++r) {
-                po[r] = cmul(p[r], o[r]);
-                u[4 * i + r] = make_float2(2.f * po[r].x - u[4 * i + r].x, 2.f * po[r].y - u[4 * i + r].y);
-            }
-            tmem_st8(t_po + 8 * i, po[0], po[1], po[2], po[3]);
+        }
+        __syncthreads();                    // the whole prefetch buffer has been read
+        if (tid == 0) {
+            bulk_load(pbuf, a.amp + (size_t)view * RNN, 65536, &mb_amp);
+            if (nview < a.n_views) bulk_load(pbuf + 65536, nsrc + 65536, 65536, &mb_hi);
         }
         tmem_wait_st();
         // ---- S3: forward 2-D FFT ----
@@ -381,31 +447,46 @@ __global__ void __launch_bounds__(RNT, 1) regfft128_kernel(const RegArgs a)
             } else {
                 __syncthreads();
             }
-            const float4 *ampv = reinterpret_cast<const float4 *>(a.amp + (size_t)view * RNN) + tid;
+            mbar_wait(&mb_amp, par);
+            const float4 *ampv = reinterpret_cast<const float4 *>(pbuf) + tid;
             const float4 *peers = a.sbuf + (((size_t)par * gridDim.x + (size_t)cl * M) * 8) * RNT + tid;
+            // peers' |F|^2 come from L2: JB registers-quads per peer are requested at once
+            constexpr int JB = (MT == 1 || MT == 2) ? 4 : 1;
+            constexpr int MP = MT ? MT : 8;
 #pragma unroll
-            for (int j = 0; j < 8; ++j) {
-                const float4 am = __ldg(ampv + j * RNT);
-                float4 S = make_float4(0.f, 0.f, 0.f, 0.f);
+            for (int j0 = 0; j0 < 8; j0 += JB) {
+                float4 pv[MP][JB];
 #pragma unroll
-                for (int mm = 0; mm < (MT ? MT : 8); ++mm) {
-                    if (mm < M) {
-                        float4 v;
-                        if (mm == m) v = make_float4(abs2_rn(u[4 * j]), abs2_rn(u[4 * j + 1]), abs2_rn(u[4 * j + 2]), abs2_rn(u[4 * j + 3]));
-                        else v = __ldcg(peers + ((size_t)mm * 8 + j) * RNT);
-                        S.x += v.x; S.y += v.y; S.z += v.z; S.w += v.w;
+                for (int mm = 0; mm < MP; ++mm)
+                    if (mm < M && mm != m) {
+#pragma unroll
+                        for (int jj = 0; jj < JB; ++jj) pv[mm][jj] = __ldcg(peers + ((size_t)mm * 8 + j0 + jj) * RNT);
                     }
-                }
-                const float Sv[4] = {S.x, S.y, S.z, S.w}, av[4] = {am.x, am.y, am.z, am.w};
 #pragma unroll
-                for (int c = 0; c < 4; ++c) {
-                    const float rs = rsqrtf(Sv[c] + a.eps);
-                    const float d = Sv[c] * rs - av[c];
-                    e0 = fmaf(d, d, e0);
-                    e1 = fmaf(av[c], av[c], e1);
-                    const float sc = av[c] * rs * cfac;
-                    u[4 * j + c].x *= sc;
-                    u[4 * j + c].y *= sc;
+                for (int jj = 0; jj < JB; ++jj) {
+                    const int j = j0 + jj;
+                    const float4 am = ampv[j * RNT];
+                    float4 S = make_float4(0.f, 0.f, 0.f, 0.f);
+#pragma unroll
+                    for (int mm = 0; mm < MP; ++mm) {
+                        if (mm < M) {
+                            float4 v;
+                            if (mm == m) v = make_float4(abs2_rn(u[4 * j]), abs2_rn(u[4 * j + 1]), abs2_rn(u[4 * j + 2]), abs2_rn(u[4 * j + 3]));
+                            else v = pv[mm][jj];
+                            S.x += v.x; S.y += v.y; S.z += v.z; S.w += v.w;
+                        }
+                    }
+                    const float Sv[4] = {S.x, S.y, S.z, S.w}, av[4] = {am.x, am.y, am.z, am.w};
+#pragma unroll
+                    for (int c = 0; c < 4; ++c) {
+                        const float rs = rsqrtf(Sv[c] + a.eps);
+                        const float d = Sv[c] * rs - av[c];
+                        e0 = fmaf(d, d, e0);
+                        e1 = fmaf(av[c], av[c], e1);
+                        const float sc = av[c] * rs * cfac;
+                        u[4 * j + c].x *= sc;
+                        u[4 * j + c].y *= sc;
+                    }
                 }
             }
         }
@@ -414,6 +495,8 @@ __global__ void __launch_bounds__(RNT, 1) regfft128_kernel(const RegArgs a)
 #pragma unroll
         for (int z = 0; z < 2; ++z) {
             __syncthreads();
+            // (z == 0) every thread is past S4: half A (sqrt(I)) is free for the next frame's rows 0..63
+            if (z == 0 && tid == 0 && nview < a.n_views) bulk_load(pbuf, nsrc, 65536, &mb_lo);
             x2_write(u, z, w, t, xb2);
             __syncthreads();
             x2_read(u, z, w, t, xb2);
