@@ -37,6 +37,8 @@ struct dm_plan {
     double beta, a_obj, a_probe, eps_f;
     int path_req, path;                  // requested / chosen (1 staged, 2 fused, 3 register-resident)
     int reg_grid;                        // path 3: number of persistent CTAs (multiple of M)
+    bool reg_sw;                         // path 3: software group barrier instead of a hardware cluster
+    int *reg_gbar;                       // path 3: [REG_MAX_CTAS] group barrier counters
     // path 4 (dm_warpfft.cuh): ring slots, phase lag (views), tasks per view and phase, persistent CTAs
     int wf_S, wf_D, wf_nA, wf_nB, wf_nC, wf_grid, wf_nw;
     int wf_lag_req;                      // 0 = derive the lag from the task counts
@@ -202,6 +204,7 @@ size_t carve(dm_plan *p, unsigned char *base)
     p->wy_d = (float2 *)take(128 * sizeof(float2));
     p->wx_d = (float2 *)take(128 * sizeof(float2));
     p->sbuf = (float4 *)take(p->N == 128 ? (size_t)2 * REG_MAX_CTAS * 8 * dmreg::RNT * sizeof(float4) : 0);
+    p->reg_gbar = (int *)take(REG_MAX_CTAS * sizeof(int));
     p->tw_d = (float2 *)take(p->N * sizeof(float2));
     p->errors = (double *)take((size_t)ERR_ROWS_CAP * (2 + p->K + p->L) * sizeof(double));
     {
@@ -299,15 +302,19 @@ template <int MT> dm_status launch_regfft_t(dm_plan *plan, cudaStream_t st, bool
     cfg.attrs = at;
     cfg.numAttrs = plan->M > 1 ? 1 : 0;
     if (query_only) {
-        int ncl = 0;
+        int ncl = 0, dev = 0, sms = 0, per = 0;
+        CU(cudaGetDevice(&dev));
+        CU(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+        CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per, kern, dmreg::RNT, dmreg::REG_SMEM_V1));
+        plan->reg_sw = false;
         if (plan->M > 1) {
             cfg.gridDim = dim3((unsigned)plan->M);
             CU(cudaOccupancyMaxActiveClusters(&ncl, kern, &cfg));
+            // a cluster of M can strand SMs (M = 4: 132 of 148 on B200); then the M CTAs of a view
+            // synchronise through a counter in L2 instead and the grid fills every SM
+            const int ncl_sw = sms * per / plan->M;
+            if (ncl_sw > ncl) { ncl = ncl_sw; plan->reg_sw = true; }
         } else {
-            int dev = 0, sms = 0, per = 0;
-            CU(cudaGetDevice(&dev));
-            CU(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
-            CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per, kern, dmreg::RNT, dmreg::REG_SMEM_V1));
             ncl = sms * per;
         }
         if (ncl < 1) return fail(plan, DM_ERR_CUDA, "register-resident kernel: no cluster of %d CTAs fits", plan->M);
@@ -324,6 +331,13 @@ template <int MT> dm_status launch_regfft_t(dm_plan *plan, cudaStream_t st, bool
     a.sbuf = plan->sbuf; a.part = plan->partA;
     a.beta = (float)plan->beta; a.eps = (float)plan->eps_f;
     cfg.gridDim = dim3((unsigned)plan->reg_grid);
+    if (plan->reg_sw) {
+        a.gbar = plan->reg_gbar;
+        CU(cudaMemsetAsync(plan->reg_gbar, 0, REG_MAX_CTAS * sizeof(int), st));
+        at[0].id = cudaLaunchAttributeCooperative;      // all CTAs resident: they wait on one another
+        at[0].val.cooperative = 1;
+        cfg.numAttrs = 1;
+    }
     CU(cudaLaunchKernelEx(&cfg, kern, a));
     return DM_OK;
 }

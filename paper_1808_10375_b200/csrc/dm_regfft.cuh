@@ -247,6 +247,7 @@ struct RegArgs {
     float4 *sbuf;               // [2][grid][8][512]  |F|^2 of every resident CTA (mode-sum exchange, L2)
     float *part;                // [grid][4]  (eF_num, eF_den, epsi_num, epsi_den) partial sums
     float beta, eps;
+    int *gbar;                  // [grid / M] software group barrier counters (NULL: hardware cluster barrier)
 };
 
 // shared memory: [prefetch buffer 128 KiB | exchange buffer | twiddles 2 KiB]
@@ -363,7 +364,8 @@ __global__ void __launch_bounds__(RNT, 1) regfft128_kernel(const RegArgs a)
         bulk_load(pbuf + 65536, src + 65536, 65536, &mb_hi);
     }
 
-    for (int view = cl; view < a.n_views; view += ncl, par ^= 1) {
+    int it = 0;
+    for (int view = cl; view < a.n_views; view += ncl, par ^= 1, ++it) {
         const int2 p0 = a.pos[view];
         float2 *psi_f = a.psi + ((size_t)view * M + m) * RNN + w * RN + t;
         const float2 *Ow = a.O + (size_t)l * a.H * a.W + (size_t)(p0.x + w) * a.W + p0.y + t;
@@ -442,8 +444,24 @@ __global__ void __launch_bounds__(RNT, 1) regfft128_kernel(const RegArgs a)
 #pragma unroll
                 for (int j = 0; j < 8; ++j)
                     mine[j * RNT] = make_float4(abs2_rn(u[4 * j]), abs2_rn(u[4 * j + 1]), abs2_rn(u[4 * j + 2]), abs2_rn(u[4 * j + 3]));
-                cluster_arrive();
-                cluster_wait();
+                if (a.gbar) {
+                    // the M CTAs of the view are not a hardware cluster (a cluster of M would leave SMs
+                    // idle): release / acquire on a counter in L2; every CTA of the grid is resident
+                    __syncthreads();
+                    if (tid == 0) {
+                        __threadfence();
+                        atomicAdd(a.gbar + cl, 1);
+                        const int want = M * (it + 1);
+                        int v;
+                        do {
+                            asm volatile("ld.acquire.gpu.global.s32 %0, [%1];\n" : "=r"(v) : "l"(a.gbar + cl) : "memory");
+                        } while (v < want);
+                    }
+                    __syncthreads();
+                } else {
+                    cluster_arrive();
+                    cluster_wait();
+                }
             } else {
                 __syncthreads();
             }
