@@ -27,6 +27,15 @@ METRIC = "dm_mode_views_per_s"
 UNIT = "mode-views/s"
 
 
+def measured_traffic(workload: str, path: int):
+    """DRAM bytes per launch of the psi-update kernel from the committed ncu --set full captures
+    (profiles/traffic.json, written by hand from the reports named there); None if not captured."""
+    p = os.path.join(ROOT, "profiles", "traffic.json")
+    if os.path.exists(p):
+        return json.load(open(p)).get(f"{workload}:path{path}", {}).get("dram_bytes_per_launch")
+    return None
+
+
 def measured_peaks():
     p = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(p):
@@ -235,7 +244,8 @@ def run_ours(args, cfg):
                    "l2": f"inputs larger than L2 (psi {MV * NN * 8 / 2**20:.0f} MiB streamed every step)"
                          if MV * NN * 8 > 2 * 126 * 2**20 else "psi fits L2: latency-bound case, no flush"},
         "roofline": {"bound": "hbm", "kernel": "psi update (S1-S6)", "achieved": achieved, "peak": peak,
-                     "unit": "GB/s", "frac": achieved / peak, "traffic": None, "peak_source": peak_src,
+                     "unit": "GB/s", "frac": achieved / peak, "traffic": measured_traffic(cfg.name, info["path"]),
+                     "peak_source": peak_src,
                      "bytes_per_launch": psi_bytes, "ms_per_launch": psi_ms},
         "iteration_roofline": {"bytes_min": bmin, "achieved_gbs": bmin / (ms_step * 1e-3) / 1e9,
                                "frac_of_measured_hbm": bmin / (ms_step * 1e-3) / 1e9 / peak},
