@@ -198,3 +198,40 @@ def rel_l2(a: np.ndarray, b: np.ndarray) -> float:
     den = np.linalg.norm(b.ravel())
     num = np.linalg.norm((a - b).ravel())
     return float(num / den) if den > 0 else float(num)
+
+
+def make_sampled_problem(cfg: DMConfig | int, sample_views, seed: int = 0) -> DMProblem:
+    """Full-size inputs for parity on SAMPLED views (tests at BASELINE.json's full sizes, where the
+    oracle cannot hold every view): positions, probe and object as in make_problem, but noise-free
+    intensities are synthesised for `sample_views` only (all other frames are zero) and the start
+    state is the near-truth one, P0 = 0.9 P_true, O0 = O_true, whose spectrum has the data's own
+    shape (an FP32-well-conditioned first step)."""
+    if isinstance(cfg, int):
+        cfg = CONFIGS[cfg]
+    rng = np.random.default_rng(seed)
+    n, h, w = cfg.N, cfg.obj_h, cfg.obj_w
+    pos = make_positions(cfg, rng)
+    amp = rng.uniform(0.8, 1.0, size=(h, w))
+    obj = [amp * np.exp(1j * _phase_field(rng, h, w, cfg.phase_sigma))]
+    for _ in range(1, cfg.L):
+        obj.append(0.3 * np.exp(1j * _phase_field(rng, h, w, cfg.phase_sigma)))
+    obj = np.stack(obj)
+    probe = make_probe(cfg)
+    inten = np.zeros((cfg.n_views, n, n), dtype=np.float32)
+    ar = np.arange(n)
+    for j in sample_views:
+        yy = pos[j, 0] + ar[:, None]
+        xx = pos[j, 1] + ar[None, :]
+        acc = np.zeros((n, n))
+        for l in range(cfg.L):
+            for k in range(cfg.K):
+                f = _fft.fft2(obj[l][yy, xx] * probe[k])
+                acc += f.real ** 2 + f.imag ** 2
+        inten[j] = acc
+    return DMProblem(
+        cfg=cfg, positions=pos, intensities=inten,
+        probe0=np.ascontiguousarray(0.9 * probe, dtype=np.complex64),
+        object0=np.ascontiguousarray(obj, dtype=np.complex64),
+        probe_true=np.ascontiguousarray(probe, dtype=np.complex64),
+        object_true=np.ascontiguousarray(obj, dtype=np.complex64),
+    )
