@@ -151,19 +151,16 @@ def run_ours(args, cfg):
     import torch
     from paper_1808_10375_b200 import dm, synth
 
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    rank = int(os.environ.get("RANK", "0"))
+    from paper_1808_10375_b200.replicas import ReplicaGroup
     local = int(os.environ.get("LOCAL_RANK", "0"))
     assert torch.cuda.is_available(), "bench.py needs a CUDA device (no CPU fallback)"
     torch.cuda.set_device(local)
-    dist = None
-    if world > 1:
-        import torch.distributed as dist
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    grp = ReplicaGroup("nccl", torch.device("cuda", local))
+    world, rank = grp.world, grp.rank
     dm.lib()
 
     # every rank reconstructs its own data set (replicas; seed = rank)
-    pr = synth.make_problem(cfg, seed=rank)
+    pr = synth.make_problem(cfg, seed=grp.seed)
     plan = dm.DMPlan(cfg.N, cfg.n_views, cfg.K, cfg.L, cfg.obj_h, cfg.obj_w, pr.positions,
                      path=args.path, **({"lag": args.lag} if args.lag else {})).alloc_workspace()
     I_h = torch.from_numpy(pr.intensities).pin_memory()
@@ -174,18 +171,7 @@ def run_ours(args, cfg):
     I_d, P_d, O_d = I_h.cuda(), P_h.cuda(), O_h.cuda()
     stream = torch.cuda.current_stream()
 
-    def barrier():
-        torch.cuda.synchronize()
-        if dist is not None:
-            dist.barrier()
-        torch.cuda.synchronize()
-
-    def max_over_ranks(x: float) -> float:
-        if dist is None:
-            return x
-        t = torch.tensor([x], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        return float(t.item())
+    barrier, max_over_ranks = grp.barrier, grp.max_over_ranks
 
     sampler = ClockSampler(local)
     sampler.start()
@@ -219,13 +205,12 @@ def run_ours(args, cfg):
     clocks = sampler.stop()
 
     if rank != 0:
-        if dist is not None:
-            dist.destroy_process_group()
+        grp.close()
         return
 
     MV, NN = cfg.mode_views, cfg.N * cfg.N
     ms_step = ms_total / args.steps
-    value = world * MV * args.steps / (ms_total * 1e-3)
+    value = grp.aggregate(MV, args.steps, ms_total)
     peak, peak_src = measured_peaks()
     psi_bytes = MV * NN * 16 + cfg.n_views * NN * 4          # psi read + write + sqrt(I) read
     psi_ms = phase_ms[0] / max(n_prof, 1)
@@ -251,7 +236,7 @@ def run_ours(args, cfg):
                                "frac_of_measured_hbm": bmin / (ms_step * 1e-3) / 1e9 / peak},
         "phase_ms_per_step": {k: float(v) / max(n_prof, 1) for k, v in
                               zip(("psi_update", "object", "probe", "errors"), phase_ms)},
-        "e2e": {"value": world * MV * e2e_steps / (ms_e2e * 1e-3), "unit": UNIT, "steps": e2e_steps,
+        "e2e": {"value": grp.aggregate(MV, e2e_steps, ms_e2e), "unit": UNIT, "steps": e2e_steps,
                 "ms_per_step": ms_e2e / e2e_steps, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                 "call": "dm_solve_host(n_iter=1): H2D intensities+P0+O0 (pinned), set_data, 1 iteration, D2H P+O"},
         "gpu_launches": info["launches_per_iter"] * args.steps,
@@ -262,8 +247,7 @@ def run_ours(args, cfg):
         line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample,
                                 "ms_per_step": ms}
     print(json.dumps(line), flush=True)
-    if dist is not None:
-        dist.destroy_process_group()
+    grp.close()
 
 
 def main():

@@ -127,6 +127,12 @@ dm_status dm_get_coverage(const dm_plan *plan, int *tile_h, int *tile_w, int32_t
  * f64[2] to HOST.  SYNCS.                                                              */
 dm_status dm_get_alphas(const dm_plan *plan, double *out_host2);
 
+/* Mode diagnostics (a probe mode is kept while its "contribution ... to the total
+ * intensity is larger than at least 1%"): the power fraction of every mode of the current
+ * state, out_host[k] = sum_r |P_k|^2 / sum_k sum_r |P_k|^2 (k < K) followed by the same for the
+ * object modes, out_host[K + l]; f64[K + L] to HOST; 0/0 := 0.  Fixed-order FP64 sums.  SYNCS.  */
+dm_status dm_get_mode_power(const dm_plan *plan, double *out_host);
+
 /* End-to-end entry with HOST buffers (what a beamline caller with data in host memory
  * does): copies intensities / probe0 / object0 HOST->DEV into a staging
  * area inside the workspace, runs dm_set_data + n_iter iterations, copies probe and object

@@ -169,6 +169,15 @@ def probe_update(positions, O, psi, P_old, alpha=0.0, real="f64"):
     return out
 
 
+def mode_power(modes):
+    """Power fraction of every mode, sum_r |X_m|^2 / sum_m sum_r |X_m|^2 (a probe mode
+    is kept while its contribution to the total intensity exceeds 1 %); 0/0 := 0.  Plain numpy, FP64."""
+    x = np.asarray(modes).astype(np.complex128)
+    p = np.array([float(np.sum(m.real ** 2 + m.imag ** 2)) for m in x])
+    t = p.sum()
+    return p / t if t > 0 else np.zeros_like(p)
+
+
 def rel_change(new, old, real="f64"):
     rt, ct = _types(real)
     new, old = _c(new, ct), _c(old, ct)

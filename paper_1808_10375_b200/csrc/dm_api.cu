@@ -58,6 +58,7 @@ struct dm_plan {
     float2 *wy_d, *wx_d;                 // path 3 twiddle tables
     float4 *sbuf;                        // path 3 mode-sum exchange (L2 resident)
     double *errors;
+    double *mode_pow;                    // [K + L] scratch of dm_get_mode_power
     float *stage_I;
     float2 *stage_P, *stage_O;
     int curP, curO;
@@ -206,6 +207,7 @@ size_t carve(dm_plan *p, unsigned char *base)
     p->sbuf = (float4 *)take(p->N == 128 ? (size_t)2 * REG_MAX_CTAS * 8 * dmreg::RNT * sizeof(float4) : 0);
     p->reg_gbar = (int *)take(REG_MAX_CTAS * sizeof(int));
     p->tw_d = (float2 *)take(p->N * sizeof(float2));
+    p->mode_pow = (double *)take((size_t)(p->K + p->L) * sizeof(double));
     p->errors = (double *)take((size_t)ERR_ROWS_CAP * (2 + p->K + p->L) * sizeof(double));
     {
         size_t sc = (size_t)p->chunk_views * p->M * NN, ring = (size_t)p->wf_S * p->M * NN;
@@ -709,7 +711,7 @@ dm_status dm_iterate(dm_plan *plan, int n_iter, void *stream)
         e.pO = plan->partO; e.nO = plan->nty * plan->ntx;
         e.K = plan->K; e.L = plan->L;
         e.row = plan->errors + (size_t)plan->rows * ncol;
-        error_finalize_kernel<<<ncol, 256, 0, st>>>(e);
+        error_finalize_kernel<<<ncol, ERR_NT, 0, st>>>(e);
         CU(cudaGetLastError());
         if (ev) CU(cudaEventRecord(ev[4], st));
         plan->curO = nO;
@@ -807,6 +809,25 @@ dm_status dm_get_alphas(const dm_plan *plan, double *out_host2)
     CU(cudaMemcpy(a, plan->alphas, sizeof a, cudaMemcpyDeviceToHost));
     out_host2[0] = a[0];
     out_host2[1] = a[1];
+    return DM_OK;
+}
+
+dm_status dm_get_mode_power(const dm_plan *plan, double *out_host)
+{
+    dm_status s = check_ready(plan, true);
+    if (s != DM_OK) return s;
+    if (!out_host) return fail(plan, DM_ERR_INVALID_ARG, "NULL output");
+    const size_t NN = (size_t)plan->N * plan->N, HW = (size_t)plan->H * plan->W;
+    CU(cudaDeviceSynchronize());
+    mode_power_kernel<<<plan->K, 1024>>>(plan->Pbuf[plan->curP], NN, plan->mode_pow);
+    mode_power_kernel<<<plan->L, 1024>>>(plan->Obuf[plan->curO], HW, plan->mode_pow + plan->K);
+    CU(cudaGetLastError());
+    CU(cudaMemcpy(out_host, plan->mode_pow, (size_t)(plan->K + plan->L) * sizeof(double), cudaMemcpyDeviceToHost));
+    double tp = 0.0, to = 0.0;
+    for (int k = 0; k < plan->K; ++k) tp += out_host[k];
+    for (int l = 0; l < plan->L; ++l) to += out_host[plan->K + l];
+    for (int k = 0; k < plan->K; ++k) out_host[k] = tp > 0.0 ? out_host[k] / tp : 0.0;
+    for (int l = 0; l < plan->L; ++l) out_host[plan->K + l] = to > 0.0 ? out_host[plan->K + l] / to : 0.0;
     return DM_OK;
 }
 

@@ -564,6 +564,23 @@ __global__ void __launch_bounds__(256) probe_finalize_kernel(
     }
 }
 
+// -------------------------------------------------------------- mode diagnostics ----
+// out[m] = sum over the n elements of mode m of |x|^2 (FP64, fixed order).
+__global__ void __launch_bounds__(1024) mode_power_kernel(const float2 *__restrict__ x, size_t n, double *__restrict__ out)
+{
+    __shared__ double sh[1024];
+    const float2 *p = x + (size_t)blockIdx.x * n;
+    double acc = 0.0;
+    for (size_t i = threadIdx.x; i < n; i += 1024) acc += (double)p[i].x * (double)p[i].x + (double)p[i].y * (double)p[i].y;
+    sh[threadIdx.x] = acc;
+    __syncthreads();
+    for (int w = 512; w > 0; w >>= 1) {
+        if ((int)threadIdx.x < w) sh[threadIdx.x] += sh[threadIdx.x + w];
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) out[blockIdx.x] = sh[0];
+}
+
 // ---------------------------------------------------------------------- errors ------
 // One CTA per column of the error row: fixed-order FP64 sums of (num, den) partial pairs,
 // value = sqrt(num/den), 0/0 := 0   (eq. (7); A10).
@@ -576,24 +593,41 @@ struct ErrArgs {
     double *row;
 };
 
-__global__ void __launch_bounds__(256) error_finalize_kernel(const ErrArgs a)
+constexpr int ERR_NT = 1024;
+
+__global__ void __launch_bounds__(ERR_NT) error_finalize_kernel(const ErrArgs a)
 {
-    __shared__ double sn[256], sd[256];
+    __shared__ double sn[ERR_NT], sd[ERR_NT];
     const int q = blockIdx.x;
     const float *p; int n, s;
     if (q == 0)            { p = a.pF; n = a.nF; s = a.sF; }
     else if (q == 1)       { p = a.pS; n = a.nS; s = a.sS; }
     else if (q < 2 + a.K)  { p = a.pP + 2 * (q - 2); n = a.nP; s = 2 * a.K; }
     else                   { p = a.pO + 2 * (q - 2 - a.K); n = a.nO; s = 2 * a.L; }
+    // fixed order: thread t sums i = t, t + NT, ... (four loads in flight), then a binary tree over t
     double num = 0.0, den = 0.0;
-    for (int i = threadIdx.x; i < n; i += 256) {
+    int i = threadIdx.x;
+    for (; i + 3 * ERR_NT < n; i += 4 * ERR_NT) {
+        float vn[4], vd[4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            vn[u] = p[(size_t)(i + u * ERR_NT) * s];
+            vd[u] = p[(size_t)(i + u * ERR_NT) * s + 1];
+        }
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            num += (double)vn[u];
+            den += (double)vd[u];
+        }
+    }
+    for (; i < n; i += ERR_NT) {
         num += (double)p[(size_t)i * s];
         den += (double)p[(size_t)i * s + 1];
     }
     sn[threadIdx.x] = num;
     sd[threadIdx.x] = den;
     __syncthreads();
-    for (int w = 128; w > 0; w >>= 1) {
+    for (int w = ERR_NT / 2; w > 0; w >>= 1) {
         if ((int)threadIdx.x < w) {
             sn[threadIdx.x] += sn[threadIdx.x + w];
             sd[threadIdx.x] += sd[threadIdx.x + w];

@@ -23,7 +23,7 @@ PARAM = {"beta": 0, "alpha_obj": 1, "alpha_probe": 2, "eps_f": 3, "path": 4, "la
 SYMBOLS = (
     "dm_plan_create", "dm_plan_set_param", "dm_plan_workspace_bytes", "dm_plan_set_workspace",
     "dm_set_data", "dm_iterate", "dm_get_probe", "dm_get_object", "dm_get_psi", "dm_get_errors",
-    "dm_set_state", "dm_get_window_table", "dm_get_coverage", "dm_get_alphas", "dm_solve_host",
+    "dm_set_state", "dm_get_window_table", "dm_get_coverage", "dm_get_alphas", "dm_get_mode_power", "dm_solve_host",
     "dm_plan_info", "dm_plan_set_profiling", "dm_get_phase_ms", "dm_host_fft2", "dm_host_fft2_path", "dm_status_string", "dm_last_error", "dm_plan_destroy",
 )
 
@@ -59,6 +59,7 @@ def lib() -> C.CDLL:
         L.dm_get_window_table.argtypes = [_vp, _vp]
         L.dm_get_coverage.argtypes = [_vp, C.POINTER(_int), C.POINTER(_int), _vp, _vp, C.POINTER(C.c_int64)]
         L.dm_get_alphas.argtypes = [_vp, _vp]
+        L.dm_get_mode_power.argtypes = [_vp, _vp]
         L.dm_solve_host.argtypes = [_vp, _vp, _vp, _vp, _int, _vp, _vp, _vp]
         L.dm_plan_info.argtypes = [_vp, C.POINTER(_int), C.POINTER(_int)]
         L.dm_plan_set_profiling.argtypes = [_vp, _int]
@@ -202,6 +203,12 @@ class DMPlan:
         out = np.zeros(2)
         self._check(self._lib.dm_get_alphas(self._h, _np_ptr(out)))
         return tuple(out)
+
+    def mode_power(self):
+        """(probe fractions [K], object fractions [L]) of the current state."""
+        out = np.zeros(self.K + self.L)
+        self._check(self._lib.dm_get_mode_power(self._h, _np_ptr(out)))
+        return out[: self.K].copy(), out[self.K:].copy()
 
     def info(self):
         p, n = _int(), _int()

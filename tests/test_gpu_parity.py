@@ -277,3 +277,17 @@ def test_mode_counts_and_ragged_shapes(dm, N, K, L, ny, nx, path):
     eg, eo = g.errors()[-1], o.errors()[-1]
     assert np.abs(eg - eo).max() <= 1e-5 * max(1.0, np.abs(eo).max())
     g.close(); o.close()
+
+
+def test_mode_power_diagnostics(dm):
+    """dm_get_mode_power against the oracle's plain definition: on an identical state (the oracle's
+    after one iteration, cast to complex64 on both sides) and after one more iteration each."""
+    pr = synth.make_problem(synth.CONFIGS[3].scaled(3, 3))
+    g, o = forced_pair(dm, pr, 1)
+    for tol in (1e-6, 1e-5):
+        gp, go = g.mode_power()
+        assert abs(gp.sum() - 1) < 1e-12 and abs(go.sum() - 1) < 1e-12
+        assert np.abs(gp - oracle.mode_power(o.probe())).max() < tol
+        assert np.abs(go - oracle.mode_power(o.object())).max() < tol
+        g.iterate(1); o.iterate(1)
+    g.close(); o.close()

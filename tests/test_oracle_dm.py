@@ -362,3 +362,18 @@ def test_create_rejects_bad_arguments():
         o.set_param("beta", 1.5)
     with pytest.raises(RuntimeError):
         o.iterate(1)                                         # no data yet
+
+
+def test_mode_power_closed_form():
+    """Mode diagnostics: the synthetic probe modes are sqrt(w_k) * roll(base), so their
+    power fractions are the weights w_k exactly; a mode scaled by c changes its share by c^2."""
+    for ci in (1, 2, 3, 4):
+        cfg = synth.CONFIGS[ci]
+        P = synth.make_probe(cfg)
+        f = oracle.mode_power(P)
+        assert np.allclose(f, np.array(cfg.weights) / sum(cfg.weights), rtol=0, atol=1e-12)
+        assert abs(f.sum() - 1.0) < 1e-14
+    x = np.ones((2, 4, 4), np.complex128)
+    x[1] *= 3j
+    assert np.allclose(oracle.mode_power(x), [0.1, 0.9])
+    assert np.all(oracle.mode_power(np.zeros((3, 2, 2))) == 0.0)
