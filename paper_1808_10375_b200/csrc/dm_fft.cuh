@@ -16,8 +16,16 @@
 
 namespace dmfft {
 
+// On the device complex add / subtract are ONE packed instruction each (Blackwell add.f32x2 /
+// fma.rn.f32x2 with a -1 multiplier: same round-to-nearest results as two scalar adds, half the
+// issue slots; the FP32 pipe still retires 128 lanes per clock).
+#if defined(__CUDA_ARCH__) && __CUDA_ARCH__ >= 1000 && !defined(DM_NO_F32X2)
+__device__ __forceinline__ float2 cadd(float2 a, float2 b) { return __fadd2_rn(a, b); }
+__device__ __forceinline__ float2 csub(float2 a, float2 b) { return __ffma2_rn(b, make_float2(-1.f, -1.f), a); }
+#else
 DM_HD float2 cadd(float2 a, float2 b) { return make_float2(a.x + b.x, a.y + b.y); }
 DM_HD float2 csub(float2 a, float2 b) { return make_float2(a.x - b.x, a.y - b.y); }
+#endif
 DM_HD float2 cmul(float2 a, float2 b) { return make_float2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x); }
 // a * conj(b)
 DM_HD float2 cmulc(float2 a, float2 b) { return make_float2(a.x * b.x + a.y * b.y, a.y * b.x - a.x * b.y); }
