@@ -137,7 +137,10 @@ dm_status dm_get_mode_power(const dm_plan *plan, double *out_host);
  * does): copies intensities / probe0 / object0 HOST->DEV into a staging
  * area inside the workspace, runs dm_set_data + n_iter iterations, copies probe and object
  * DEV->HOST, and SYNCS.  out_probe_host / out_object_host may be NULL.  Needs the
- * workspace (which includes the staging area).                                          */
+ * workspace (which includes the staging area).  The intensities travel in 8 chunks on an
+ * internal copy stream while the set-up kernels that do not need them (psi = P0*O0, the
+ * frozen regularisers) run on `stream`; pass pinned host memory for the copies to be
+ * asynchronous.  Results are bit-identical to the device-pointer calls.                 */
 dm_status dm_solve_host(dm_plan *plan, const float *intensities_host, const float *probe0_host,
                         const float *object0_host, int n_iter, float *out_probe_host,
                         float *out_object_host, void *stream);

@@ -69,6 +69,11 @@ struct dm_plan {
     bool profiling;
     std::vector<cudaEvent_t> ev;         // 5 events per profiled iteration
     int ev_iters;
+    // dm_solve_host: the intensities travel on a second stream, in chunks, under the set-up kernels
+    cudaStream_t copy_st;
+    cudaEvent_t ev_begin, ev_chunk[8];
+    bool copy_ready;
+    int tables_path;                     // path whose tables / twiddles are on the device (0: none)
     mutable std::string err;
 };
 
@@ -516,7 +521,7 @@ dm_status dm_plan_create(dm_plan **out, int N, int n_views, int K, int L, int ob
     p->path_req = 0; p->path = 0; p->wf_lag_req = 0;
     p->ws = nullptr; p->ws_bytes = 0;
     p->curP = p->curO = 0; p->has_data = false; p->rows = 0;
-    p->profiling = false; p->ev_iters = 0;
+    p->profiling = false; p->ev_iters = 0; p->copy_ready = false; p->tables_path = 0;
     build_tables(p);
     plan_geometry(p);
     p->need_bytes = carve(p, nullptr);
@@ -565,10 +570,18 @@ dm_status dm_plan_set_workspace(dm_plan *plan, void *dev, size_t bytes)
     plan->ws_bytes = bytes;
     carve(plan, (unsigned char *)dev);
     plan->has_data = false;
+    plan->tables_path = 0;
     return DM_OK;
 }
 
-dm_status dm_set_data(dm_plan *plan, const float *intensities, const float *probe0, const float *object0, void *stream)
+} // extern "C"
+
+namespace {
+// dm_set_data proper.  n_chunks > 0 (dm_solve_host): `intensities` arrives in n_chunks pieces of
+// whole views, piece c being complete once chunk_ev[c] has fired; sqrt(I) is then formed piece by
+// piece AFTER the kernels that do not need the data, so those run under the host-to-device copy.
+dm_status set_data_impl(dm_plan *plan, const float *intensities, const float *probe0, const float *object0, void *stream,
+                        const cudaEvent_t *chunk_ev, int n_chunks)
 {
     dm_status s = check_ready(plan, false);
     if (s != DM_OK) return s;
@@ -582,7 +595,10 @@ dm_status dm_set_data(dm_plan *plan, const float *intensities, const float *prob
     plan->path = path;
     cudaStream_t st = (cudaStream_t)stream;
     const size_t NN = (size_t)plan->N * plan->N, HW = (size_t)plan->H * plan->W;
-    // spectrum layout of the chosen path (where sqrt(I) has to sit)
+    // spectrum layout of the chosen path (where sqrt(I) has to sit), twiddles and integer tables: uploaded once
+    // per workspace and path (host-to-device copies of pageable memory would otherwise queue behind the
+    // intensities of dm_solve_host on the copy engine)
+    if (plan->tables_path != path) {
     plan->spec.assign(NN, 0);
     if (path == 3) {
         for (int tid = 0; tid < dmreg::RNT; ++tid)
@@ -640,12 +656,15 @@ dm_status dm_set_data(dm_plan *plan, const float *intensities, const float *prob
         CU(cudaMemcpyAsync(plan->tile_views_d, plan->tile_views.data(), plan->tile_views.size() * sizeof(int32_t), cudaMemcpyHostToDevice, st));
     CU(cudaMemcpyAsync(plan->spec_d, plan->spec.data(), plan->spec.size() * sizeof(int32_t), cudaMemcpyHostToDevice, st));
     CU(cudaMemcpyAsync(plan->tw_d, plan->tw.data(), plan->tw.size() * sizeof(float), cudaMemcpyHostToDevice, st));
+    CU(cudaStreamSynchronize(st));              // pageable host sources
+    plan->tables_path = path;
+    }
     plan->curP = plan->curO = 0;
     CU(cudaMemcpyAsync(plan->Pbuf[0], probe0, plan->K * NN * sizeof(float2), cudaMemcpyDeviceToDevice, st));
     CU(cudaMemcpyAsync(plan->Obuf[0], object0, plan->L * HW * sizeof(float2), cudaMemcpyDeviceToDevice, st));
     CU(cudaMemsetAsync(plan->alphas, 0, 2 * sizeof(float), st));
     const size_t total = (size_t)plan->n_views * NN;
-    amp_permute_kernel<<<148 * 8, 256, 0, st>>>(plan->N, intensities, plan->spec_d, plan->amp, total);
+    if (n_chunks <= 0) amp_permute_kernel<<<148 * 8, 256, 0, st>>>(plan->N, intensities, plan->spec_d, plan->amp, total);
     psi_init_kernel<<<dim3((unsigned)((NN + 1023) / 1024), (unsigned)(plan->n_views * plan->M)), 256, 0, st>>>(
         plan->N, plan->K, plan->L, plan->H, plan->W, plan->pos_d, plan->Pbuf[0], plan->Obuf[0], plan->psi);
     CU(cudaGetLastError());
@@ -658,9 +677,25 @@ dm_status dm_set_data(dm_plan *plan, const float *intensities, const float *prob
     if (s != DM_OK) return s;
     max_scale_kernel<<<1, 1024, 0, st>>>(plan->den_tmp, NN, (float)plan->a_probe, plan->alphas + 1);
     CU(cudaGetLastError());
+    for (int c = 0; c < n_chunks; ++c) {
+        const int v0 = (int)((long long)plan->n_views * c / n_chunks), v1 = (int)((long long)plan->n_views * (c + 1) / n_chunks);
+        if (v1 == v0) continue;
+        CU(cudaStreamWaitEvent(st, chunk_ev[c], 0));
+        amp_permute_kernel<<<148 * 8, 256, 0, st>>>(plan->N, intensities + (size_t)v0 * NN, plan->spec_d,
+                                                    plan->amp + (size_t)v0 * NN, (size_t)(v1 - v0) * NN);
+    }
+    CU(cudaGetLastError());
     plan->has_data = true;
     plan->rows = 0;
     return DM_OK;
+}
+} // namespace
+
+extern "C" {
+
+dm_status dm_set_data(dm_plan *plan, const float *intensities, const float *probe0, const float *object0, void *stream)
+{
+    return set_data_impl(plan, intensities, probe0, object0, stream, nullptr, 0);
 }
 
 dm_status dm_iterate(dm_plan *plan, int n_iter, void *stream)
@@ -840,11 +875,28 @@ dm_status dm_solve_host(dm_plan *plan, const float *intensities_host, const floa
     if (!intensities_host || !probe0_host || !object0_host) return fail(plan, DM_ERR_INVALID_ARG, "NULL data pointer");
     cudaStream_t st = (cudaStream_t)stream;
     const size_t NN = (size_t)plan->N * plan->N, HW = (size_t)plan->H * plan->W;
-    CU(cudaMemcpyAsync(plan->stage_I, intensities_host, (size_t)plan->n_views * NN * sizeof(float), cudaMemcpyHostToDevice, st));
+    constexpr int NCH = 8;
+    if (!plan->copy_ready) {
+        CU(cudaStreamCreateWithFlags(&plan->copy_st, cudaStreamNonBlocking));
+        CU(cudaEventCreateWithFlags(&plan->ev_begin, cudaEventDisableTiming));
+        for (int c = 0; c < NCH; ++c) CU(cudaEventCreateWithFlags(&plan->ev_chunk[c], cudaEventDisableTiming));
+        plan->copy_ready = true;
+    }
+    // P0, O0 (small) first on the caller's stream; the intensities in NCH chunks on the copy stream,
+    // which starts once everything already queued on `st` (earlier readers of the staging area) is done
+    CU(cudaEventRecord(plan->ev_begin, st));
+    CU(cudaStreamWaitEvent(plan->copy_st, plan->ev_begin, 0));
     CU(cudaMemcpyAsync(plan->stage_P, probe0_host, plan->K * NN * sizeof(float2), cudaMemcpyHostToDevice, st));
     CU(cudaMemcpyAsync(plan->stage_O, object0_host, plan->L * HW * sizeof(float2), cudaMemcpyHostToDevice, st));
+    for (int c = 0; c < NCH; ++c) {
+        const size_t v0 = (size_t)((long long)plan->n_views * c / NCH), v1 = (size_t)((long long)plan->n_views * (c + 1) / NCH);
+        if (v1 > v0)
+            CU(cudaMemcpyAsync(plan->stage_I + v0 * NN, intensities_host + v0 * NN, (v1 - v0) * NN * sizeof(float),
+                               cudaMemcpyHostToDevice, plan->copy_st));
+        CU(cudaEventRecord(plan->ev_chunk[c], plan->copy_st));
+    }
     plan->has_data = false;
-    s = dm_set_data(plan, plan->stage_I, (const float *)plan->stage_P, (const float *)plan->stage_O, stream);
+    s = set_data_impl(plan, plan->stage_I, (const float *)plan->stage_P, (const float *)plan->stage_O, stream, plan->ev_chunk, NCH);
     if (s != DM_OK) return s;
     s = dm_iterate(plan, n_iter, stream);
     if (s != DM_OK) return s;
@@ -1109,6 +1161,11 @@ void dm_plan_destroy(dm_plan *plan)
 {
     if (!plan) return;
     for (cudaEvent_t e : plan->ev) cudaEventDestroy(e);
+    if (plan->copy_ready) {
+        cudaStreamDestroy(plan->copy_st);
+        cudaEventDestroy(plan->ev_begin);
+        for (int c = 0; c < 8; ++c) cudaEventDestroy(plan->ev_chunk[c]);
+    }
     delete plan;
 }
 
