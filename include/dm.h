@@ -61,10 +61,18 @@ typedef enum {
                                  path (DM_ERR_UNSUPPORTED at dm_set_data unless N = 128),
                                  4 = force the view-pipelined warp-FFT path (any N; the
                                  default for N >= 256)                                       */
-    DM_PARAM_LAG = 5          /* path 4: views between the row, column and inverse-row phases
+    DM_PARAM_LAG = 5,         /* path 4: views between the row, column and inverse-row phases
                                  of one view (integer >= 1; 0 = derive from the task counts,
                                  default).  Sizes the scratch ring: set before
                                  dm_plan_set_workspace (INVALID_ARG afterwards)              */
+    DM_PARAM_PRECISION = 6    /* 0 = FP32 / complex64 (default, the tuned paths); 1 = FP64 /
+                                 complex128 validation mode: the whole iteration in the
+                                 paper's own precision with plain kernels and
+                                 the definition's summation orders -- for long free-running
+                                 comparisons, not for speed.  Inputs and getters stay
+                                 float32 / complex64 (converted at the boundary); the error
+                                 table is f64 either way.  Needs a larger workspace: set
+                                 before dm_plan_set_workspace (INVALID_ARG afterwards)       */
 } dm_param;
 
 /* Build the plan (HOST only, no CUDA call): validates, copies `positions` (HOST,

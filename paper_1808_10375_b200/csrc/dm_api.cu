@@ -10,6 +10,7 @@
 
 #include "../../include/dm.h"
 #include "dm_kernels.cuh"
+#include "dm_fp64.cuh"
 
 namespace {
 
@@ -73,6 +74,10 @@ struct dm_plan {
     cudaStream_t copy_st;
     cudaEvent_t ev_begin, ev_chunk[8];
     bool copy_ready;
+    // DM_PARAM_PRECISION = 1: the FP64 validation mode (dm_fp64.cuh)
+    int precision;
+    double2 *psi64, *scr64, *P64[2], *O64[2], *tw64;
+    double *amp64, *den64, *alphas64, *partF64, *partS64, *partP64, *partO64;
     int tables_path;                     // path whose tables / twiddles are on the device (0: none)
     mutable std::string err;
 };
@@ -220,6 +225,20 @@ size_t carve(dm_plan *p, unsigned char *base)
     }
     p->wf_cnt = (int *)take((1 + 3 * (size_t)p->n_views) * sizeof(int));
     p->wf_tw_d = (float2 *)take((size_t)p->N * sizeof(float2));
+    if (p->precision == 1) {
+        p->psi64 = (double2 *)take(MV * NN * sizeof(double2));
+        p->scr64 = (double2 *)take(MV * NN * sizeof(double2));
+        for (int i = 0; i < 2; ++i) p->P64[i] = (double2 *)take(p->K * NN * sizeof(double2));
+        for (int i = 0; i < 2; ++i) p->O64[i] = (double2 *)take(p->L * HW * sizeof(double2));
+        p->tw64 = (double2 *)take((size_t)p->N / 2 * sizeof(double2));
+        p->amp64 = (double *)take((size_t)p->n_views * NN * sizeof(double));
+        p->den64 = (double *)take((HW > NN ? HW : NN) * sizeof(double));
+        p->alphas64 = (double *)take(2 * sizeof(double));
+        p->partF64 = (double *)take((size_t)p->n_views * (NN / 256) * 2 * sizeof(double));
+        p->partS64 = (double *)take(MV * p->N * 2 * sizeof(double));
+        p->partP64 = (double *)take((size_t)(NN / 256) * p->K * 2 * sizeof(double));
+        p->partO64 = (double *)take((size_t)p->nty * p->ntx * p->L * 2 * sizeof(double));
+    }
     p->stage_I = (float *)take((size_t)p->n_views * NN * sizeof(float));
     p->stage_P = (float2 *)take(p->K * NN * sizeof(float2));
     p->stage_O = (float2 *)take(p->L * HW * sizeof(float2));
@@ -521,7 +540,7 @@ dm_status dm_plan_create(dm_plan **out, int N, int n_views, int K, int L, int ob
     p->path_req = 0; p->path = 0; p->wf_lag_req = 0;
     p->ws = nullptr; p->ws_bytes = 0;
     p->curP = p->curO = 0; p->has_data = false; p->rows = 0;
-    p->profiling = false; p->ev_iters = 0; p->copy_ready = false; p->tables_path = 0;
+    p->profiling = false; p->ev_iters = 0; p->copy_ready = false; p->tables_path = 0; p->precision = 0;
     build_tables(p);
     plan_geometry(p);
     p->need_bytes = carve(p, nullptr);
@@ -540,6 +559,12 @@ dm_status dm_plan_set_param(dm_plan *plan, dm_param which, double v)
     case DM_PARAM_ALPHA_PROBE: if (v < 0) break; plan->a_probe = v; return DM_OK;
     case DM_PARAM_EPS_F: if (v < 0) break; plan->eps_f = v; return DM_OK;
     case DM_PARAM_PATH: if (v != 0 && v != 1 && v != 2 && v != 3 && v != 4) break; plan->path_req = (int)v; return DM_OK;
+    case DM_PARAM_PRECISION:
+        if (v != 0 && v != 1) break;
+        if (plan->ws) return fail(plan, DM_ERR_INVALID_ARG, "the precision sizes the workspace: set it before dm_plan_set_workspace");
+        plan->precision = (int)v;
+        plan->need_bytes = carve(plan, nullptr);
+        return DM_OK;
     case DM_PARAM_LAG:
         if (v < 0 || v > 4096 || v != (double)(int)v) break;
         if (plan->ws) return fail(plan, DM_ERR_INVALID_ARG, "the phase lag sizes the workspace: set it before dm_plan_set_workspace");
@@ -577,6 +602,105 @@ dm_status dm_plan_set_workspace(dm_plan *plan, void *dev, size_t bytes)
 } // extern "C"
 
 namespace {
+constexpr int CONV_GRID = 148 * 8;
+
+dm64::Args args64(const dm_plan *p)
+{
+    dm64::Args a;
+    memset(&a, 0, sizeof a);
+    a.N = p->N; a.logN = 0;
+    while ((1 << a.logN) < p->N) ++a.logN;
+    a.n_views = p->n_views; a.K = p->K; a.L = p->L; a.H = p->H; a.W = p->W;
+    a.pos = p->pos_d; a.P = p->P64[p->curP]; a.O = p->O64[p->curO];
+    a.psi = p->psi64; a.scratch = p->scr64; a.amp = p->amp64; a.tw = p->tw64;
+    a.beta = p->beta; a.eps = p->eps_f;
+    a.partF = p->partF64; a.partS = p->partS64;
+    return a;
+}
+
+dm_status launch_object64(dm_plan *plan, cudaStream_t st, const double2 *P, const double2 *O_old, double2 *O_new, double *den_out)
+{
+    dm64::object64_kernel<<<plan->nty * plan->ntx, OBJ_TH * OBJ_TW, 0, st>>>(
+        plan->N, plan->K, plan->L, plan->H, plan->W, OBJ_TH, OBJ_TW, plan->pos_d, plan->tile_ptr_d, plan->tile_views_d, P,
+        plan->psi64, O_old, O_new, plan->alphas64, plan->partO64, den_out);
+    CU(cudaGetLastError());
+    return DM_OK;
+}
+
+dm_status launch_probe64(dm_plan *plan, cudaStream_t st, const double2 *O, const double2 *P_old, double2 *P_new, double *den_out)
+{
+    const size_t NN = (size_t)plan->N * plan->N;
+    dm64::probe64_kernel<<<dim3((unsigned)(NN / 256), (unsigned)plan->K), 256, 0, st>>>(
+        plan->N, plan->K, plan->L, plan->n_views, plan->H, plan->W, plan->pos_d, O, plan->psi64, P_old, P_new,
+        plan->alphas64, plan->partP64, den_out);
+    CU(cudaGetLastError());
+    return DM_OK;
+}
+
+// FP64 mode: state from float32 / complex64 inputs (widened exactly), psi = P0 * O0, frozen regularisers
+dm_status set_data64(dm_plan *plan, const float *intensities, const float *probe0, const float *object0, cudaStream_t st)
+{
+    const size_t NN = (size_t)plan->N * plan->N, HW = (size_t)plan->H * plan->W;
+    std::vector<double> tw((size_t)plan->N);
+    for (int n = 0; n < plan->N / 2; ++n) {
+        const double ang = -2.0 * M_PI * (double)n / (double)plan->N;
+        tw[2 * n] = std::cos(ang);
+        tw[2 * n + 1] = std::sin(ang);
+    }
+    CU(cudaMemcpyAsync(plan->tw64, tw.data(), tw.size() * sizeof(double), cudaMemcpyHostToDevice, st));
+    CU(cudaStreamSynchronize(st));
+    plan->curP = plan->curO = 0;
+    dm64::f2d_kernel<<<CONV_GRID, 256, 0, st>>>(probe0, (double *)plan->P64[0], 2 * plan->K * NN, 0);
+    dm64::f2d_kernel<<<CONV_GRID, 256, 0, st>>>(object0, (double *)plan->O64[0], 2 * plan->L * HW, 0);
+    dm64::f2d_kernel<<<CONV_GRID, 256, 0, st>>>(intensities, plan->amp64, (size_t)plan->n_views * NN, 1);
+    CU(cudaMemsetAsync(plan->alphas64, 0, 2 * sizeof(double), st));
+    dm64::psi_init64_kernel<<<dim3((unsigned)((NN + 1023) / 1024), (unsigned)(plan->n_views * plan->M)), 256, 0, st>>>(
+        plan->N, plan->K, plan->L, plan->H, plan->W, plan->pos_d, plan->P64[0], plan->O64[0], plan->psi64);
+    CU(cudaGetLastError());
+    dm_status s = launch_object64(plan, st, plan->P64[0], plan->O64[0], plan->O64[1], plan->den64);
+    if (s != DM_OK) return s;
+    dm64::max_scale64_kernel<<<1, 1024, 0, st>>>(plan->den64, HW, plan->a_obj, plan->alphas64);
+    s = launch_probe64(plan, st, plan->O64[0], plan->P64[0], plan->P64[1], plan->den64);
+    if (s != DM_OK) return s;
+    dm64::max_scale64_kernel<<<1, 1024, 0, st>>>(plan->den64, NN, plan->a_probe, plan->alphas64 + 1);
+    CU(cudaGetLastError());
+    return DM_OK;
+}
+
+// FP64 mode: one DM iteration (order of DESIGN.md §1: psi update, object, probe, error row)
+dm_status iterate64(dm_plan *plan, cudaStream_t st)
+{
+    const int N = plan->N;
+    const size_t NN = (size_t)N * N;
+    const unsigned lines = (unsigned)((size_t)plan->n_views * plan->M * N);
+    const size_t sm_rows = (size_t)N * sizeof(double2) + (size_t)N * sizeof(double), sm_cols = (size_t)N * sizeof(double2);
+    dm64::Args a = args64(plan);
+    dm64::rows64_kernel<true><<<lines, N / 2, sm_rows, st>>>(a);
+    dm64::cols64_kernel<false><<<lines, N / 2, sm_cols, st>>>(a);
+    dm64::modulus64_kernel<<<dim3((unsigned)(NN / 256), (unsigned)plan->n_views), 256, 0, st>>>(a);
+    dm64::cols64_kernel<true><<<lines, N / 2, sm_cols, st>>>(a);
+    dm64::rows64_kernel<false><<<lines, N / 2, sm_rows, st>>>(a);
+    CU(cudaGetLastError());
+    const int nO = 1 - plan->curO, nP = 1 - plan->curP;
+    dm_status s = launch_object64(plan, st, plan->P64[plan->curP], plan->O64[plan->curO], plan->O64[nO], nullptr);
+    if (s != DM_OK) return s;
+    s = launch_probe64(plan, st, plan->O64[nO], plan->P64[plan->curP], plan->P64[nP], nullptr);
+    if (s != DM_OK) return s;
+    dm64::Err64 e;
+    e.pF = plan->partF64; e.nF = (int)(plan->n_views * (NN / 256));
+    e.pS = plan->partS64; e.nS = (int)lines;
+    e.pP = plan->partP64; e.nP = (int)(NN / 256);
+    e.pO = plan->partO64; e.nO = plan->nty * plan->ntx;
+    e.K = plan->K; e.L = plan->L;
+    e.row = plan->errors + (size_t)plan->rows * (2 + plan->K + plan->L);
+    dm64::err64_finalize_kernel<<<2 + plan->K + plan->L, 1024, 0, st>>>(e);
+    CU(cudaGetLastError());
+    plan->curO = nO;
+    plan->curP = nP;
+    plan->rows++;
+    return DM_OK;
+}
+
 // dm_set_data proper.  n_chunks > 0 (dm_solve_host): `intensities` arrives in n_chunks pieces of
 // whole views, piece c being complete once chunk_ev[c] has fired; sqrt(I) is then formed piece by
 // piece AFTER the kernels that do not need the data, so those run under the host-to-device copy.
@@ -588,6 +712,7 @@ dm_status set_data_impl(dm_plan *plan, const float *intensities, const float *pr
     if (!intensities || !probe0 || !object0) return fail(plan, DM_ERR_INVALID_ARG, "NULL data pointer");
     int path = plan->path_req;
     if (path == 0) path = plan->N == 128 ? 3 : (plan->N < 128 ? 2 : 4);
+    if (plan->precision == 1) path = 64;         // FP64 validation mode: its own plain kernels
     if (path == 2 && plan->N > 128)
         return fail(plan, DM_ERR_UNSUPPORTED, "fused per-frame path needs N <= 128 (N = %d)", plan->N);
     if (path == 3 && plan->N != 128)
@@ -659,6 +784,14 @@ dm_status set_data_impl(dm_plan *plan, const float *intensities, const float *pr
     CU(cudaStreamSynchronize(st));              // pageable host sources
     plan->tables_path = path;
     }
+    if (plan->precision == 1) {
+        for (int c = 0; c < n_chunks; ++c) CU(cudaStreamWaitEvent(st, chunk_ev[c], 0));
+        s = set_data64(plan, intensities, probe0, object0, st);
+        if (s != DM_OK) return s;
+        plan->has_data = true;
+        plan->rows = 0;
+        return DM_OK;
+    }
     plan->curP = plan->curO = 0;
     CU(cudaMemcpyAsync(plan->Pbuf[0], probe0, plan->K * NN * sizeof(float2), cudaMemcpyDeviceToDevice, st));
     CU(cudaMemcpyAsync(plan->Obuf[0], object0, plan->L * HW * sizeof(float2), cudaMemcpyDeviceToDevice, st));
@@ -707,6 +840,11 @@ dm_status dm_iterate(dm_plan *plan, int n_iter, void *stream)
         return fail(plan, DM_ERR_WORKSPACE, "error table holds %d rows; call dm_set_data to reset", ERR_ROWS_CAP);
     cudaStream_t st = (cudaStream_t)stream;
     const int ncol = 2 + plan->K + plan->L;
+    for (int it = 0; it < n_iter && plan->precision == 1; ++it) {
+        s = iterate64(plan, st);
+        if (s != DM_OK) return s;
+    }
+    if (plan->precision == 1) return DM_OK;
     for (int it = 0; it < n_iter; ++it) {
         cudaEvent_t *ev = nullptr;
         if (plan->profiling && plan->ev_iters < PROF_MAX_ITERS) {
@@ -761,6 +899,12 @@ dm_status dm_get_probe(const dm_plan *plan, float *out_dev, void *stream)
     dm_status s = check_ready(plan, true);
     if (s != DM_OK) return s;
     if (!out_dev) return fail(plan, DM_ERR_INVALID_ARG, "NULL output");
+    if (plan->precision == 1) {
+        dm64::d2f_kernel<<<CONV_GRID, 256, 0, (cudaStream_t)stream>>>((const double *)plan->P64[plan->curP], out_dev,
+                                                                        2 * (size_t)plan->K * plan->N * plan->N);
+        CU(cudaGetLastError());
+        return DM_OK;
+    }
     CU(cudaMemcpyAsync(out_dev, plan->Pbuf[plan->curP], (size_t)plan->K * plan->N * plan->N * sizeof(float2),
                        cudaMemcpyDeviceToDevice, (cudaStream_t)stream));
     return DM_OK;
@@ -771,6 +915,12 @@ dm_status dm_get_object(const dm_plan *plan, float *out_dev, void *stream)
     dm_status s = check_ready(plan, true);
     if (s != DM_OK) return s;
     if (!out_dev) return fail(plan, DM_ERR_INVALID_ARG, "NULL output");
+    if (plan->precision == 1) {
+        dm64::d2f_kernel<<<CONV_GRID, 256, 0, (cudaStream_t)stream>>>((const double *)plan->O64[plan->curO], out_dev,
+                                                                        2 * (size_t)plan->L * plan->H * plan->W);
+        CU(cudaGetLastError());
+        return DM_OK;
+    }
     CU(cudaMemcpyAsync(out_dev, plan->Obuf[plan->curO], (size_t)plan->L * plan->H * plan->W * sizeof(float2),
                        cudaMemcpyDeviceToDevice, (cudaStream_t)stream));
     return DM_OK;
@@ -781,6 +931,12 @@ dm_status dm_get_psi(const dm_plan *plan, float *out_dev, void *stream)
     dm_status s = check_ready(plan, true);
     if (s != DM_OK) return s;
     if (!out_dev) return fail(plan, DM_ERR_INVALID_ARG, "NULL output");
+    if (plan->precision == 1) {
+        dm64::d2f_kernel<<<CONV_GRID, 256, 0, (cudaStream_t)stream>>>((const double *)plan->psi64, out_dev,
+                                                                        2 * (size_t)plan->n_views * plan->M * plan->N * plan->N);
+        CU(cudaGetLastError());
+        return DM_OK;
+    }
     CU(cudaMemcpyAsync(out_dev, plan->psi, (size_t)plan->n_views * plan->M * plan->N * plan->N * sizeof(float2),
                        cudaMemcpyDeviceToDevice, (cudaStream_t)stream));
     return DM_OK;
@@ -804,6 +960,13 @@ dm_status dm_set_state(dm_plan *plan, const float *probe_dev, const float *objec
     if (s != DM_OK) return s;
     cudaStream_t st = (cudaStream_t)stream;
     const size_t NN = (size_t)plan->N * plan->N, HW = (size_t)plan->H * plan->W;
+    if (plan->precision == 1) {
+        if (probe_dev) dm64::f2d_kernel<<<CONV_GRID, 256, 0, st>>>(probe_dev, (double *)plan->P64[plan->curP], 2 * plan->K * NN, 0);
+        if (object_dev) dm64::f2d_kernel<<<CONV_GRID, 256, 0, st>>>(object_dev, (double *)plan->O64[plan->curO], 2 * plan->L * HW, 0);
+        if (psi_dev) dm64::f2d_kernel<<<CONV_GRID, 256, 0, st>>>(psi_dev, (double *)plan->psi64, 2 * (size_t)plan->n_views * plan->M * NN, 0);
+        CU(cudaGetLastError());
+        return DM_OK;
+    }
     if (probe_dev) CU(cudaMemcpyAsync(plan->Pbuf[plan->curP], probe_dev, plan->K * NN * sizeof(float2), cudaMemcpyDeviceToDevice, st));
     if (object_dev) CU(cudaMemcpyAsync(plan->Obuf[plan->curO], object_dev, plan->L * HW * sizeof(float2), cudaMemcpyDeviceToDevice, st));
     if (psi_dev) CU(cudaMemcpyAsync(plan->psi, psi_dev, (size_t)plan->n_views * plan->M * NN * sizeof(float2), cudaMemcpyDeviceToDevice, st));
@@ -839,8 +1002,12 @@ dm_status dm_get_alphas(const dm_plan *plan, double *out_host2)
     dm_status s = check_ready(plan, true);
     if (s != DM_OK) return s;
     if (!out_host2) return fail(plan, DM_ERR_INVALID_ARG, "NULL output");
-    float a[2];
     CU(cudaDeviceSynchronize());
+    if (plan->precision == 1) {
+        CU(cudaMemcpy(out_host2, plan->alphas64, 2 * sizeof(double), cudaMemcpyDeviceToHost));
+        return DM_OK;
+    }
+    float a[2];
     CU(cudaMemcpy(a, plan->alphas, sizeof a, cudaMemcpyDeviceToHost));
     out_host2[0] = a[0];
     out_host2[1] = a[1];
@@ -854,6 +1021,10 @@ dm_status dm_get_mode_power(const dm_plan *plan, double *out_host)
     if (!out_host) return fail(plan, DM_ERR_INVALID_ARG, "NULL output");
     const size_t NN = (size_t)plan->N * plan->N, HW = (size_t)plan->H * plan->W;
     CU(cudaDeviceSynchronize());
+    if (plan->precision == 1) {     // the FP32 state buffers are unused in this mode: park the rounded state there
+        dm64::d2f_kernel<<<CONV_GRID, 256>>>((const double *)plan->P64[plan->curP], (float *)plan->Pbuf[plan->curP], 2 * plan->K * NN);
+        dm64::d2f_kernel<<<CONV_GRID, 256>>>((const double *)plan->O64[plan->curO], (float *)plan->Obuf[plan->curO], 2 * plan->L * HW);
+    }
     mode_power_kernel<<<plan->K, 1024>>>(plan->Pbuf[plan->curP], NN, plan->mode_pow);
     mode_power_kernel<<<plan->L, 1024>>>(plan->Obuf[plan->curO], HW, plan->mode_pow + plan->K);
     CU(cudaGetLastError());
@@ -900,6 +1071,10 @@ dm_status dm_solve_host(dm_plan *plan, const float *intensities_host, const floa
     if (s != DM_OK) return s;
     s = dm_iterate(plan, n_iter, stream);
     if (s != DM_OK) return s;
+    if (plan->precision == 1) {     // round the FP64 state into the FP32 state buffers (unused in this mode)
+        dm64::d2f_kernel<<<CONV_GRID, 256, 0, st>>>((const double *)plan->P64[plan->curP], (float *)plan->Pbuf[plan->curP], 2 * plan->K * NN);
+        dm64::d2f_kernel<<<CONV_GRID, 256, 0, st>>>((const double *)plan->O64[plan->curO], (float *)plan->Obuf[plan->curO], 2 * plan->L * HW);
+    }
     if (out_probe_host)
         CU(cudaMemcpyAsync(out_probe_host, plan->Pbuf[plan->curP], plan->K * NN * sizeof(float2), cudaMemcpyDeviceToHost, st));
     if (out_object_host)
@@ -937,10 +1112,11 @@ dm_status dm_plan_info(const dm_plan *plan, int *path, int *launches_per_iter)
 {
     if (!plan) return DM_ERR_INVALID_ARG;
     int p = plan->path ? plan->path : (plan->path_req ? plan->path_req : (plan->N == 128 ? 3 : (plan->N < 128 ? 2 : 4)));
+    if (plan->precision == 1) p = 64;
     if (path) *path = p;
     if (launches_per_iter) {
         const int chunks = (plan->n_views + plan->chunk_views - 1) / plan->chunk_views;
-        *launches_per_iter = (p >= 2 ? 1 : 3 * chunks) + 4;
+        *launches_per_iter = p == 64 ? 8 : (p >= 2 ? 1 : 3 * chunks) + 4;
     }
     return DM_OK;
 }

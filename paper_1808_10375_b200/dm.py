@@ -17,7 +17,7 @@ LIB_PATH = os.path.join(_HERE, "libdm_b200.so")
 DM_OK = 0
 STATUS = {0: "DM_OK", 1: "DM_ERR_INVALID_ARG", 2: "DM_ERR_OUT_OF_BOUNDS", 3: "DM_ERR_UNSUPPORTED",
           4: "DM_ERR_NO_DATA", 5: "DM_ERR_WORKSPACE", 6: "DM_ERR_CUDA"}
-PARAM = {"beta": 0, "alpha_obj": 1, "alpha_probe": 2, "eps_f": 3, "path": 4, "lag": 5}
+PARAM = {"beta": 0, "alpha_obj": 1, "alpha_probe": 2, "eps_f": 3, "path": 4, "lag": 5, "precision": 6}
 
 # every symbol include/dm.h declares (tests check the library exports exactly these)
 SYMBOLS = (

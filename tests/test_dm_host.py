@@ -76,6 +76,17 @@ def test_params_and_call_order(dm):
             p.set_param(name, v)
         assert e.value.status == 1
     assert p.workspace_bytes() > 2 * 64 * 64 * 8
+    w32 = p.workspace_bytes()
+    p.set_param("precision", 1)                     # FP64 validation mode: larger workspace (psi + spectra in c128)
+    assert p.workspace_bytes() >= w32 + 2 * 2 * 64 * 64 * 16
+    p.set_param("precision", 0)
+    assert p.workspace_bytes() == w32
+    p.set_param("lag", 3)
+    p.set_param("lag", 0)
+    for name, v in (("precision", 2), ("precision", -1), ("lag", -1), ("lag", 1.5)):
+        with pytest.raises(dm.DMError) as e:
+            p.set_param(name, v)
+        assert e.value.status == 1
     with pytest.raises(dm.DMError) as e:            # no workspace yet
         p._check(p._lib.dm_iterate(p._h, 1, None))
     assert e.value.status == 5
@@ -90,6 +101,10 @@ def test_params_and_call_order(dm):
     with pytest.raises(dm.DMError) as e:
         p._check(p._lib.dm_iterate(p._h, 1, None))
     assert e.value.status == 4
+    for name in ("precision", "lag"):                # both size the workspace: refused once it is set
+        with pytest.raises(dm.DMError) as e:
+            p.set_param(name, 1)
+        assert e.value.status == 1
     p.close()
 
 
