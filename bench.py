@@ -107,13 +107,16 @@ def sample_cfg(cfg, target_mode_views: int):
     return cfg.scaled(ny, nx)
 
 
-def time_oracle(cfg, steps: int, warmup: int, target_mode_views: int):
+def time_oracle(cfg, steps: int, warmup: int, target_mode_views: int, threads: int = 0):
     """The oracle as it stands (oracle/dm_oracle.c, FP64, OpenMP over views / pixels) on the host
     cores, on a bounded sample of the workload.  Returns (mode-views/s, ms/step, cores, sample text)."""
     import oracle
     from paper_1808_10375_b200 import synth
     sc = sample_cfg(cfg, target_mode_views)
     pr = synth.make_problem(sc)
+    all_threads = oracle.num_threads()
+    if threads:
+        oracle.set_num_threads(threads)
     o = oracle.OracleDM(sc.N, sc.K, sc.L, sc.obj_h, sc.obj_w, pr.positions)
     o.set_data(pr.intensities, pr.probe0, pr.object0)
     o.iterate(warmup)
@@ -122,6 +125,8 @@ def time_oracle(cfg, steps: int, warmup: int, target_mode_views: int):
     dt = time.perf_counter() - t0
     cores = oracle.num_threads()
     o.close()
+    if threads:
+        oracle.set_num_threads(all_threads)
     sample = (f"{sc.name}: {sc.ny}x{sc.nx} raster ({sc.n_views} views, {sc.mode_views} mode-views) of "
               f"{cfg.name}, same N={sc.N} K={sc.K} L={sc.L}, {steps} iteration(s) after {warmup} warm-up")
     return sc.mode_views * steps / dt, 1e3 * dt / steps, cores, sample
@@ -246,6 +251,10 @@ def run_ours(args, cfg):
         v, ms, cores, sample = time_oracle(cfg, 1, 1, args.ref_mode_views)
         line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample,
                                 "ms_per_step": ms}
+        # one host thread, smaller sample: context for the paper's single-core figure
+        v1, ms1, c1, sample1 = time_oracle(cfg, 1, 0, max(64, args.ref_mode_views // 16), threads=1)
+        line["cpu_baseline_1thread"] = {"value": v1, "unit": UNIT, "cores": c1, "kind": "oracle", "sample": sample1,
+                                        "ms_per_step": ms1}
     print(json.dumps(line), flush=True)
     grp.close()
 
