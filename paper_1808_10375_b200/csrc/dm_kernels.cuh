@@ -487,7 +487,40 @@ __global__ void __launch_bounds__(PRB_NT) probe_partial_kernel(
     for (int k = 0; k < KT; ++k) num[k] = make_float4(0.f, 0.f, 0.f, 0.f);
     float den0 = 0.f, den1 = 0.f;
     const size_t HW = (size_t)H * W;
-    for (int j = j0; j < j1; ++j) {
+    int j = j0;
+    if (L == 1) {
+        // L = 1 (every config but c3): UV views per step, all of their psi / O loads issued before the
+        // first use (memory-level parallelism); the sums keep the order j ascending
+        constexpr int UV = KT <= 2 ? 4 : 2;
+        for (; j + UV <= j1; j += UV) {
+            float4 sv[UV][KT];
+            float2 o0[UV], o1[UV];
+#pragma unroll
+            for (int u = 0; u < UV; ++u) {
+                const int2 p0 = __ldg(pos + j + u);
+                const float2 *ob = O + (size_t)(p0.x + ry) * W + p0.y + rx;
+                o0[u] = __ldg(ob);
+                o1[u] = __ldg(ob + 1);
+#pragma unroll
+                for (int k = 0; k < KT; ++k)
+                    sv[u][k] = __ldg(reinterpret_cast<const float4 *>(psi + ((size_t)(j + u) * KT + k) * NN + r));
+            }
+#pragma unroll
+            for (int u = 0; u < UV; ++u) {
+                den0 += cabs2(o0[u]);
+                den1 += cabs2(o1[u]);
+#pragma unroll
+                for (int k = 0; k < KT; ++k) {
+                    const float4 s = sv[u][k];
+                    num[k].x += o0[u].x * s.x + o0[u].y * s.y;
+                    num[k].y += o0[u].x * s.y - o0[u].y * s.x;
+                    num[k].z += o1[u].x * s.z + o1[u].y * s.w;
+                    num[k].w += o1[u].x * s.w - o1[u].y * s.z;
+                }
+            }
+        }
+    }
+    for (; j < j1; ++j) {
         const int2 p0 = __ldg(pos + j);
         const float2 *ob = O + (size_t)(p0.x + ry) * W + p0.y + rx;
         const float2 *ps = psi + (size_t)j * KT * L * NN + r;
