@@ -260,6 +260,13 @@ __global__ void __launch_bounds__(32 * WF_MAXW, 2) wf_dataflow_kernel(const WfAr
             // ---- spectrum rows of one column group, one mode: lane t holds y = t + 32 s ----
             active = (w < GPT * M) && (cg < NG);
             if (active) {
+                // sqrt(I) of this column group comes from HBM and is only needed after the forward FFT:
+                // start it towards L2 now (no registers held), one mode's warp per group does it
+                if (m_b == 0) {
+                    const float4 *ampv = reinterpret_cast<const float4 *>(a.amp + (size_t)view * NN) + (size_t)cg * 256 + t;
+#pragma unroll
+                    for (int j = 0; j < 8; ++j) asm volatile("prefetch.global.L2 [%0];\n" :: "l"(ampv + j * 32));
+                }
                 const float2 *src = slot + (size_t)m_b * NN + (size_t)cg * N * G + (size_t)t * G;
 #pragma unroll
                 for (int s = 0; s < RX; ++s)
