@@ -384,11 +384,11 @@ template <int N> dm_status launch_wf_t(dm_plan *plan, cudaStream_t st, bool quer
 {
     auto kern = dmwf::wf_dataflow_kernel<N>;
     const int nt = 32 * plan->wf_nw;
-    const int smem = plan->wf_nw * dmwf::WF_XBUF + (N / 32) * 32 * (int)sizeof(float2);
+    const int smem = plan->wf_nw * dmwf::WF_XBUF + (N / 32) * 32 * (int)sizeof(float2) + (plan->wf_nw / plan->M) * 4096;
     static bool attr_done = false;
     if (!attr_done) {
         CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                dmwf::WF_MAXW * dmwf::WF_XBUF + (N / 32) * 32 * (int)sizeof(float2)));
+                                dmwf::WF_MAXW * dmwf::WF_XBUF + (N / 32) * 32 * (int)sizeof(float2) + dmwf::WF_MAXW * 4096));
         attr_done = true;
     }
     if (query_only) {

@@ -180,6 +180,8 @@ __global__ void __launch_bounds__(32 * WF_MAXW, 2) wf_dataflow_kernel(const WfAr
     const int M = a.K * a.L;
     unsigned char *wbuf = smem + w * WF_XBUF;                 // exchange buffer; doubles as the |F|^2 buffer
     float2 *s_tw = reinterpret_cast<float2 *>(smem + NW * WF_XBUF);       // [RX][32]
+    // sqrt(I) of the task's column groups, staged by cp.async while the forward FFT runs: [NW / M][8][32] float4
+    float4 *s_amp = reinterpret_cast<float4 *>(smem + NW * WF_XBUF + RX * 32 * sizeof(float2));
     for (int i = tid; i < RX * 32; i += blockDim.x) s_tw[i] = a.tw[i];
     const int T = a.nA + a.nB + a.nC;
     const int total = (a.n_views + 2 * a.D) * T;
@@ -261,11 +263,14 @@ __global__ void __launch_bounds__(32 * WF_MAXW, 2) wf_dataflow_kernel(const WfAr
             active = (w < GPT * M) && (cg < NG);
             if (active) {
                 // sqrt(I) of this column group comes from HBM and is only needed after the forward FFT:
-                // start it towards L2 now (no registers held), one mode's warp per group does it
+                // copy it asynchronously into shared memory now (no registers held), one warp per group
                 if (m_b == 0) {
                     const float4 *ampv = reinterpret_cast<const float4 *>(a.amp + (size_t)view * NN) + (size_t)cg * 256 + t;
+                    const unsigned dst = (unsigned)__cvta_generic_to_shared(s_amp + (size_t)(w / M) * 256 + t);
 #pragma unroll
-                    for (int j = 0; j < 8; ++j) asm volatile("prefetch.global.L2 [%0];\n" :: "l"(ampv + j * 32));
+                    for (int j = 0; j < 8; ++j)
+                        asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" :: "r"(dst + j * 512), "l"(ampv + j * 32) : "memory");
+                    asm volatile("cp.async.commit_group;\n" ::: "memory");
                 }
                 const float2 *src = slot + (size_t)m_b * NN + (size_t)cg * N * G + (size_t)t * G;
 #pragma unroll
@@ -296,14 +301,15 @@ __global__ void __launch_bounds__(32 * WF_MAXW, 2) wf_dataflow_kernel(const WfAr
                 for (int j = 0; j < 8; ++j)
                     mine[j * 32] = make_float4(abs2_rn(u[4 * j]), abs2_rn(u[4 * j + 1]), abs2_rn(u[4 * j + 2]), abs2_rn(u[4 * j + 3]));
             }
+            if (active && m_b == 0) asm volatile("cp.async.wait_all;\n" ::: "memory");
             __syncthreads();
             if (active) {
-                const float4 *ampv = reinterpret_cast<const float4 *>(a.amp + (size_t)view * NN) + (size_t)cg * 256 + t;
+                const float4 *ampv = s_amp + (size_t)(w / M) * 256 + t;
                 const unsigned char *peers = smem + (size_t)(w - m_b) * WF_XBUF;
                 const float cfac = 1.f / (float)NN;
 #pragma unroll
                 for (int j = 0; j < 8; ++j) {
-                    const float4 am = __ldg(ampv + j * 32);
+                    const float4 am = ampv[j * 32];
                     float4 S = make_float4(0.f, 0.f, 0.f, 0.f);
 #pragma unroll
                     for (int mm = 0; mm < WF_MAXW; ++mm)
