@@ -286,6 +286,12 @@ __global__ void __launch_bounds__(32 * WF_MAXW, 2) wf_dataflow_kernel(const WfAr
             // ---- scaled spectrum rows back from scratch: lane a = (g, k1), register k2 ----
             active = rgi < M * NG;
             if (active) {
+                // psi_old is needed after the inverse FFT and may have left L2 since phase A read it
+                {
+                    const char *rows = reinterpret_cast<const char *>(a.psi + ((size_t)view * M + m_ac) * NN + (size_t)y0 * N);
+#pragma unroll
+                    for (int i = 0; i < 2; ++i) asm volatile("prefetch.global.L2 [%0];\n" :: "l"(rows + (size_t)(t + 32 * i) * 128));
+                }
                 const float2 *src = slot + (size_t)m_ac * NN + sidx;
 #pragma unroll
                 for (int k2 = 0; k2 < 32; ++k2) u[k2] = __ldcg(src + scratch_index<N>(0, RX * k2));
