@@ -397,6 +397,22 @@ __global__ void __launch_bounds__(32 * WF_MAXW, 2) wf_dataflow_kernel(const WfAr
             }
             if (t == 0) { red[w] = e0; red[WF_MAXW + w] = e1; }
         }
+        // thread 0 looks at the next task's dependency counter NOW: the round trip of that acquire load
+        // overlaps with the barrier and the release below instead of following them
+        const int *dep = nullptr;
+        int want = 0, seen = 0;
+        bool early = false;
+        if (tid == 0 && nxt < total) {
+            int nphase, nsub, nview;
+            decode(nxt, nphase, nsub, nview);
+            if (nview >= 0 && nview < a.n_views) {
+                early = true;
+                if (nphase == 0) { if (nview >= a.S) { dep = a.cntC + nview - a.S; want = a.nC; } }
+                else if (nphase == 1) { dep = a.cntA + nview; want = a.nA; }
+                else { dep = a.cntB + nview; want = a.nB; }
+                if (dep) asm volatile("ld.acquire.gpu.global.s32 %0, [%1];\n" : "=r"(seen) : "l"(dep) : "memory");
+            }
+        }
         __syncthreads();
         if (tid == 0) {
             if (phase != 0) {
@@ -408,7 +424,12 @@ __global__ void __launch_bounds__(32 * WF_MAXW, 2) wf_dataflow_kernel(const WfAr
             }
             __threadfence();
             atomicAdd((phase == 0 ? a.cntA : phase == 1 ? a.cntB : a.cntC) + view, 1);
-            s_task[buf ^ 1] = resolve(nxt);
+            if (early) {
+                if (dep && seen < want) spin_until(dep, want);
+                s_task[buf ^ 1] = nxt;
+            } else {
+                s_task[buf ^ 1] = resolve(nxt);
+            }
         }
         __syncthreads();
     }
