@@ -173,8 +173,8 @@ __global__ void __launch_bounds__(32 * WF_MAXW, 2) wf_dataflow_kernel(const WfAr
 {
     constexpr int RX = N / 32, G = 32 / RX, NN = N * N, NG = N / G;     // NG: column groups = row groups per frame
     extern __shared__ __align__(16) unsigned char smem[];
-    __shared__ int s_task[2];
-    __shared__ float red[2 * WF_MAXW];
+    __shared__ int s_task[2], s_go[2];
+    __shared__ float red2[2][2 * WF_MAXW];
 
     const int tid = threadIdx.x, w = tid >> 5, t = tid & 31, NW = blockDim.x >> 5;
     const int M = a.K * a.L;
@@ -225,6 +225,7 @@ __global__ void __launch_bounds__(32 * WF_MAXW, 2) wf_dataflow_kernel(const WfAr
         float2 u[32];
         bool active;
         float e0 = 0.f, e1 = 0.f;
+        float *red = red2[buf];
         // A / C geometry: row group rgi of the view -> frame m, rows y0 .. y0 + G - 1
         const int rgi = sub * NW + w;
         const int m_ac = rgi / NG, y0 = (rgi % NG) * G;
@@ -413,7 +414,16 @@ __global__ void __launch_bounds__(32 * WF_MAXW, 2) wf_dataflow_kernel(const WfAr
                 if (dep) asm volatile("ld.acquire.gpu.global.s32 %0, [%1];\n" : "=r"(seen) : "l"(dep) : "memory");
             }
         }
+        // if the next task can start (the common case), publish it with the barrier that ends this one:
+        // the other warps go on while thread 0 writes the partial sums and releases the completion count
+        if (tid == 0) {
+            // (pays with many warps per CTA; with 2 or 3 the warp of thread 0 would be the straggler of the next task)
+            const bool go = NW >= 6 && early && (dep == nullptr || seen >= want);
+            s_go[buf] = go;
+            if (go) s_task[buf ^ 1] = nxt;
+        }
         __syncthreads();
+        const bool go = s_go[buf] != 0;
         if (tid == 0) {
             if (phase != 0) {
                 float s0 = 0.f, s1 = 0.f;
@@ -424,14 +434,16 @@ __global__ void __launch_bounds__(32 * WF_MAXW, 2) wf_dataflow_kernel(const WfAr
             }
             __threadfence();
             atomicAdd((phase == 0 ? a.cntA : phase == 1 ? a.cntB : a.cntC) + view, 1);
-            if (early) {
-                if (dep && seen < want) spin_until(dep, want);
-                s_task[buf ^ 1] = nxt;
-            } else {
-                s_task[buf ^ 1] = resolve(nxt);
+            if (!go) {
+                if (early) {
+                    if (dep) spin_until(dep, want);
+                    s_task[buf ^ 1] = nxt;
+                } else {
+                    s_task[buf ^ 1] = resolve(nxt);
+                }
             }
         }
-        __syncthreads();
+        if (!go) __syncthreads();
     }
 }
 
