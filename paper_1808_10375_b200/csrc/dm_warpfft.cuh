@@ -242,7 +242,7 @@ __global__ void __launch_bounds__(32 * WF_MAXW, 2) wf_dataflow_kernel(const WfAr
                 const float2 *Pk = a.P + (size_t)k * NN + (size_t)y0 * N + t;
                 const float2 *Ow = a.O + (size_t)l * a.H * a.W + (size_t)(p0.x + y0) * a.W + p0.y + t;
 #pragma unroll
-                for (int i = 0; i < 32; ++i) u[i] = psi_f[(i / RX) * N + (i % RX) * 32];
+                for (int i = 0; i < 32; ++i) u[i] = __ldcs(psi_f + (i / RX) * N + (i % RX) * 32);   // streamed once: keep L1 for P and O
 #pragma unroll
                 for (int h = 0; h < 2; ++h) {
                     float2 p[16], o[16];
