@@ -144,6 +144,24 @@ __device__ __forceinline__ void spin_until(const int *cnt, int want)
     }
 }
 
+// 256-bit (one full 32-byte sector per lane) L2-only load / store of four adjacent complex values
+__device__ __forceinline__ void ldcg256(const float2 *p, float2 &a, float2 &b, float2 &c, float2 &d)
+{
+    unsigned r0, r1, r2, r3, r4, r5, r6, r7;
+    asm volatile("ld.global.cg.v8.b32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];\n"
+                 : "=r"(r0), "=r"(r1), "=r"(r2), "=r"(r3), "=r"(r4), "=r"(r5), "=r"(r6), "=r"(r7) : "l"(p) : "memory");
+    a = make_float2(__uint_as_float(r0), __uint_as_float(r1));
+    b = make_float2(__uint_as_float(r2), __uint_as_float(r3));
+    c = make_float2(__uint_as_float(r4), __uint_as_float(r5));
+    d = make_float2(__uint_as_float(r6), __uint_as_float(r7));
+}
+__device__ __forceinline__ void stcg256(float2 *p, float2 a, float2 b, float2 c, float2 d)
+{
+    asm volatile("st.global.cg.v8.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};\n"
+                 :: "l"(p), "r"(__float_as_uint(a.x)), "r"(__float_as_uint(a.y)), "r"(__float_as_uint(b.x)), "r"(__float_as_uint(b.y)),
+                    "r"(__float_as_uint(c.x)), "r"(__float_as_uint(c.y)), "r"(__float_as_uint(d.x)), "r"(__float_as_uint(d.y)) : "memory");
+}
+
 __device__ __forceinline__ float abs2_rn(float2 f) { return __fmaf_rn(f.y, f.y, __fmul_rn(f.x, f.x)); }
 
 // forward / inverse 1-D FFT of the warp's G lines (registers <-> registers)
@@ -275,13 +293,20 @@ __global__ void __launch_bounds__(32 * WF_MAXW, 2) wf_dataflow_kernel(const WfAr
                 }
                 const float2 *src = slot + (size_t)m_b * NN + (size_t)cg * N * G + (size_t)t * G;
 #pragma unroll
-                for (int s = 0; s < RX; ++s)
+                for (int s = 0; s < RX; ++s) {
+                    if (G >= 4) {
 #pragma unroll
-                    for (int c = 0; c < G; c += 2) {
-                        const float4 v = __ldcg(reinterpret_cast<const float4 *>(src + (size_t)s * 32 * G + c));
-                        u[c * RX + s] = make_float2(v.x, v.y);
-                        u[(c + 1) * RX + s] = make_float2(v.z, v.w);
+                        for (int c = 0; c + 3 < G; c += 4)
+                            ldcg256(src + (size_t)s * 32 * G + c, u[c * RX + s], u[(c + 1) * RX + s], u[(c + 2) * RX + s], u[(c + 3) * RX + s]);
+                    } else {
+#pragma unroll
+                        for (int c = 0; c < G; c += 2) {
+                            const float4 v = __ldcg(reinterpret_cast<const float4 *>(src + (size_t)s * 32 * G + c));
+                            u[c * RX + s] = make_float2(v.x, v.y);
+                            u[(c + 1) * RX + s] = make_float2(v.z, v.w);
+                        }
                     }
+                }
             }
         } else {
             // ---- scaled spectrum rows back from scratch: lane a = (g, k1), register k2 ----
@@ -353,11 +378,18 @@ __global__ void __launch_bounds__(32 * WF_MAXW, 2) wf_dataflow_kernel(const WfAr
             if (active) {
                 float2 *dst = slot + (size_t)m_b * NN + (size_t)cg * N * G + (size_t)t * G;
 #pragma unroll
-                for (int s = 0; s < RX; ++s)
+                for (int s = 0; s < RX; ++s) {
+                    if (G >= 4) {
 #pragma unroll
-                    for (int c = 0; c < G; c += 2)
-                        __stcg(reinterpret_cast<float4 *>(dst + (size_t)s * 32 * G + c),
-                               make_float4(u[c * RX + s].x, u[c * RX + s].y, u[(c + 1) * RX + s].x, u[(c + 1) * RX + s].y));
+                        for (int c = 0; c + 3 < G; c += 4)
+                            stcg256(dst + (size_t)s * 32 * G + c, u[c * RX + s], u[(c + 1) * RX + s], u[(c + 2) * RX + s], u[(c + 3) * RX + s]);
+                    } else {
+#pragma unroll
+                        for (int c = 0; c < G; c += 2)
+                            __stcg(reinterpret_cast<float4 *>(dst + (size_t)s * 32 * G + c),
+                                   make_float4(u[c * RX + s].x, u[c * RX + s].y, u[(c + 1) * RX + s].x, u[(c + 1) * RX + s].y));
+                    }
+                }
             }
         } else {
             // ---- S6: psi_new = psi_old + beta (G - P O) ----
