@@ -335,12 +335,13 @@ __global__ void __launch_bounds__(32 * WF_MAXW, 2) wf_dataflow_kernel(const WfAr
             }
             if (active && m_b == 0) asm volatile("cp.async.wait_all;\n" ::: "memory");
             __syncthreads();
+            // reduce-scatter: the M warps of a column group share the 8 register rows j; the warp that owns row j
+            // sums |F|^2 of all modes for it, forms the scale amp / sqrt(S) and leaves it where sqrt(I) was
             if (active) {
-                const float4 *ampv = s_amp + (size_t)(w / M) * 256 + t;
+                float4 *ampv = s_amp + (size_t)(w / M) * 256 + t;
                 const unsigned char *peers = smem + (size_t)(w - m_b) * WF_XBUF;
                 const float cfac = 1.f / (float)NN;
-#pragma unroll
-                for (int j = 0; j < 8; ++j) {
+                for (int j = m_b; j < 8; j += M) {
                     const float4 am = ampv[j * 32];
                     float4 S = make_float4(0.f, 0.f, 0.f, 0.f);
 #pragma unroll
@@ -350,20 +351,30 @@ __global__ void __launch_bounds__(32 * WF_MAXW, 2) wf_dataflow_kernel(const WfAr
                             S.x += v.x; S.y += v.y; S.z += v.z; S.w += v.w;
                         }
                     const float Sv[4] = {S.x, S.y, S.z, S.w}, av[4] = {am.x, am.y, am.z, am.w};
+                    float sc[4];
 #pragma unroll
                     for (int c = 0; c < 4; ++c) {
                         const float rs = rsqrtf(Sv[c] + a.eps);
                         const float d = Sv[c] * rs - av[c];
                         e0 = fmaf(d, d, e0);
                         e1 = fmaf(av[c], av[c], e1);
-                        const float sc = av[c] * rs * cfac;
-                        u[4 * j + c].x *= sc;
-                        u[4 * j + c].y *= sc;
+                        sc[c] = av[c] * rs * cfac;
                     }
+                    ampv[j * 32] = make_float4(sc[0], sc[1], sc[2], sc[3]);
                 }
-                if (m_b != 0) { e0 = 0.f; e1 = 0.f; }
             }
-            __syncthreads();            // every warp has read the |F|^2 buffers before they serve as exchange buffers again
+            __syncthreads();            // scales complete; every warp has read the |F|^2 buffers (they serve as exchange buffers again)
+            if (active) {
+                const float4 *scv = s_amp + (size_t)(w / M) * 256 + t;
+#pragma unroll
+                for (int j = 0; j < 8; ++j) {
+                    const float4 sc = scv[j * 32];
+                    u[4 * j].x *= sc.x; u[4 * j].y *= sc.x;
+                    u[4 * j + 1].x *= sc.y; u[4 * j + 1].y *= sc.y;
+                    u[4 * j + 2].x *= sc.z; u[4 * j + 2].y *= sc.z;
+                    u[4 * j + 3].x *= sc.w; u[4 * j + 3].y *= sc.w;
+                }
+            }
         }
         // ---- inverse FFT (B: along y, C: along x) ----
         if (phase != 0 && active) warp_fft_inv<RX>(u, s_tw, t, wbuf);
