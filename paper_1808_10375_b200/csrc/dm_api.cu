@@ -165,10 +165,10 @@ void plan_geometry(dm_plan *p)
     p->wf_nC = p->wf_nA;
     p->wf_nB = (NG + GPT - 1) / GPT;
     const int T = p->wf_nA + p->wf_nB + p->wf_nC;
-    // lag: a phase starts on a view once ~2 x (resident CTAs) tasks have been queued behind its inputs
-    // (measured on B200: c3 lag 4 and c1 lag 60 beat half those lags by 10 %; psi + ring still fit L2)
+    // lag: a phase starts on a view once ~1.6 x (resident CTAs) tasks have been queued behind its inputs
+    // (measured on B200 at the end of round 1: c3 is fastest at 3-4 views, c4 at 2; a longer lag only pushes psi out of L2)
     const int resident = 148 * (16 / p->wf_nw);
-    int D = p->wf_lag_req > 0 ? p->wf_lag_req : (int)((2.0 * resident + T - 1) / T);
+    int D = p->wf_lag_req > 0 ? p->wf_lag_req : (int)((1.6 * resident + T - 1) / T);
     if (D < 1) D = 1;
     p->wf_D = D;
     p->wf_S = 2 * D + 4;
