@@ -262,11 +262,11 @@ __global__ void __launch_bounds__(32 * WF_MAXW, 2) wf_dataflow_kernel(const WfAr
 #pragma unroll
                 for (int i = 0; i < 32; ++i) u[i] = __ldcs(psi_f + (i / RX) * N + (i % RX) * 32);   // streamed once: keep L1 for P and O
 #pragma unroll
-                for (int h = 0; h < 4; ++h) {
-                    float2 p[8], o[8];
+                for (int h = 0; h < 2; ++h) {
+                    float2 p[16], o[16];
 #pragma unroll
-                    for (int i = 0; i < 8; ++i) {
-                        const int e = 8 * h + i;
+                    for (int i = 0; i < 16; ++i) {
+                        const int e = 16 * h + i;
                         p[i] = __ldg(Pk + (e / RX) * N + (e % RX) * 32);
                         o[i] = __ldg(Ow + (size_t)(e / RX) * a.W + (e % RX) * 32);
                     }
@@ -377,24 +377,7 @@ __global__ void __launch_bounds__(32 * WF_MAXW, 2) wf_dataflow_kernel(const WfAr
             }
         }
         // ---- inverse FFT (B: along y, C: along x) ----
-        if (phase != 0 && active) {
-            dmreg::dft32<true>(u);
-            xt_write(u, t, wbuf);
-            __syncwarp();
-            xt_read(u, t, wbuf);
-            __syncwarp();
-            if (phase == 2) {
-                // the exchange buffer is free from here on: psi_old (8 KiB per warp, possibly out of L2 by now)
-                // is copied into it asynchronously while the last register stage runs
-                const char *rows = reinterpret_cast<const char *>(a.psi + ((size_t)view * M + m_ac) * NN + (size_t)y0 * N);
-                const unsigned dst = (unsigned)__cvta_generic_to_shared(wbuf) + t * 16;
-#pragma unroll
-                for (int i = 0; i < 16; ++i)
-                    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" :: "r"(dst + i * 512), "l"(rows + (size_t)(i * 32 + t) * 16) : "memory");
-                asm volatile("cp.async.commit_group;\n" ::: "memory");
-            }
-            stage1_inv<RX>(u, s_tw, t);
-        }
+        if (phase != 0 && active) warp_fft_inv<RX>(u, s_tw, t, wbuf);
         // ---- stores ----
         if (phase == 0) {
             if (active) {
@@ -426,27 +409,22 @@ __global__ void __launch_bounds__(32 * WF_MAXW, 2) wf_dataflow_kernel(const WfAr
                 float2 *psi_f = a.psi + ((size_t)view * M + m_ac) * NN + (size_t)y0 * N + t;
                 const float2 *Pk = a.P + (size_t)k * NN + (size_t)y0 * N + t;
                 const float2 *Ow = a.O + (size_t)l * a.H * a.W + (size_t)(p0.x + y0) * a.W + p0.y + t;
-                const float2 *olds = reinterpret_cast<const float2 *>(wbuf) + t;    // psi_old rows, staged above
 #pragma unroll
-                for (int h = 0; h < 2; ++h) {
-                    float2 p[16], o[16];
+                for (int h = 0; h < 4; ++h) {
+                    float2 p[8], o[8], old[8];
 #pragma unroll
-                    for (int i = 0; i < 16; ++i) {
-                        const int e = 16 * h + i;
+                    for (int i = 0; i < 8; ++i) {
+                        const int e = 8 * h + i;
+                        old[i] = __ldcs(psi_f + (e / RX) * N + (e % RX) * 32);
                         p[i] = __ldg(Pk + (e / RX) * N + (e % RX) * 32);
                         o[i] = __ldg(Ow + (size_t)(e / RX) * a.W + (e % RX) * 32);
-                    }
-                    if (h == 0) {
-                        asm volatile("cp.async.wait_all;\n" ::: "memory");
-                        __syncwarp();
                     }
 #pragma unroll
                     for (int i = 0; i < 8; ++i) {
                         const int e = 8 * h + i;
                         const float2 po = cmul(p[i], o[i]);
-                        const float2 old = olds[(e / RX) * N + (e % RX) * 32];
                         const float tx = u[e].x - po.x, ty = u[e].y - po.y;
-                        const float2 nw = make_float2(fmaf(a.beta, tx, old.x), fmaf(a.beta, ty, old.y));
+                        const float2 nw = make_float2(fmaf(a.beta, tx, old[i].x), fmaf(a.beta, ty, old[i].y));
                         e0 = fmaf(tx, tx, fmaf(ty, ty, e0));
                         e1 = fmaf(nw.x, nw.x, fmaf(nw.y, nw.y, e1));
                         __stcs(psi_f + (e / RX) * N + (e % RX) * 32, nw);
