@@ -3,8 +3,10 @@
   python bench.py [--gpus N] [--steps K] [--warmup W] [--config I] [--impl ours|reference]
 
 A "step" is one whole DM iteration (psi update S1-S6, object S7, probe S8, error row S9 of
-DESIGN.md) over one synthetic fly-scan data set shaped like BASELINE.json config I (default
-configs[1]: 2500 views of 128x128, K=2).  Prints ONE JSON line (contract in DESIGN.md
+DESIGN.md) over one synthetic fly-scan data set shaped like BASELINE.json config I.  The headline
+workload is the largest single-GPU config (default configs[3]: 4096 views of 256x256, K=4, L=2;
+BASELINE.json's metric names no config); the other single-GPU configs (1, 2, 4) are measured in the
+same run and reported under "per_config".  Prints ONE JSON line (contract in DESIGN.md
 "Measurement").  N > 1 (torchrun): independent replicas, one per GPU, no data-path collective
 (north_star: the path is single-GPU).
 """
@@ -27,13 +29,37 @@ METRIC = "dm_mode_views_per_s"
 UNIT = "mode-views/s"
 
 
-def measured_traffic(workload: str, path: int):
-    """DRAM bytes per launch of the psi-update kernel from the committed ncu --set full captures
-    (profiles/traffic.json, written by hand from the reports named there); None if not captured."""
+def csrc_digest() -> str:
+    """sha256 over the CUDA sources, in file-name order: ties a stored ncu number to the kernels it was taken on."""
+    import glob
+    import hashlib
+    h = hashlib.sha256()
+    for f in sorted(glob.glob(os.path.join(ROOT, "paper_1808_10375_b200", "csrc", "*"))):
+        h.update(os.path.basename(f).encode())
+        h.update(open(f, "rb").read())
+    return h.hexdigest()[:16]
+
+
+def measured_traffic(workload: str, path: int, lag: int):
+    """DRAM bytes per launch of the psi-update kernel (dram__bytes_read.sum + dram__bytes_write.sum) from the
+    committed ncu capture of exactly these kernels: profiles/traffic.json keeps, per workload and path, the bytes,
+    the digest of csrc/ they were captured on and path 4's lag.  Returns (bytes, provenance); (None, why) when no
+    capture matches the sources and launch parameters of this run -- a stale number is never reported."""
     p = os.path.join(ROOT, "profiles", "traffic.json")
-    if os.path.exists(p):
-        return json.load(open(p)).get(f"{workload}:path{path}", {}).get("dram_bytes_per_launch")
-    return None
+    if not os.path.exists(p):
+        return None, "no capture"
+    e = json.load(open(p)).get(f"{workload}:path{path}")
+    if not e:
+        return None, "no capture for this workload / path"
+    if e.get("csrc_digest") != csrc_digest():
+        return None, f"capture {e.get('source')} was taken on other kernel sources (digest {e.get('csrc_digest')})"
+    if path == 4 and e.get("lag") != lag:
+        return None, f"capture was taken at lag {e.get('lag')}, this run uses {lag}"
+    return e["dram_bytes_per_launch"], {"file": "profiles/traffic.json", "source": e.get("source"),
+                                         "csrc_digest": e.get("csrc_digest"), "kind": "committed ncu capture, not measured in this run"}
+
+
+NOMINAL_HBM_GBS = 8000.0      # north_star / SURVEY.md 8(d): "~8 TB/s"
 
 
 def measured_peaks():
@@ -152,6 +178,61 @@ def run_reference(args, cfg):
     print(json.dumps(line), flush=True)
 
 
+def measure_device_arm(dm, synth, torch, grp, cfg, pr, steps, warmup, path, lag, stream):
+    """Device-resident arm on one config: inputs already in HBM, `steps` whole DM iterations timed with CUDA
+    events on the launching stream after `warmup` untimed ones.  Returns (plan, host tensors, result dict)."""
+    plan = dm.DMPlan(cfg.N, cfg.n_views, cfg.K, cfg.L, cfg.obj_h, cfg.obj_w, pr.positions,
+                     path=path, **({"lag": lag} if lag else {})).alloc_workspace()
+    I_h = torch.from_numpy(pr.intensities).pin_memory()
+    P_h = torch.from_numpy(pr.probe0).pin_memory()
+    O_h = torch.from_numpy(pr.object0).pin_memory()
+    I_d, P_d, O_d = I_h.cuda(), P_h.cuda(), O_h.cuda()
+    plan.set_data(I_d, P_d, O_d)
+    del I_d
+    plan.iterate(warmup)
+    plan.set_profiling(True)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    grp.barrier()
+    e0.record(stream)
+    plan.iterate(steps)
+    e1.record(stream)
+    grp.barrier()
+    ms_total = grp.max_over_ranks(e0.elapsed_time(e1))
+    phase_ms, n_prof = plan.phase_ms()
+    plan.set_profiling(False)
+    info, geo = plan.info(), plan.geometry()
+
+    MV, NN = cfg.mode_views, cfg.N * cfg.N
+    ms_step = ms_total / steps
+    peak, peak_src = measured_peaks()
+    psi_bytes = MV * NN * 16 + cfg.n_views * NN * 4          # psi read + write + sqrt(I) read (DESIGN.md)
+    psi_ms = phase_ms[0] / max(n_prof, 1)
+    achieved = psi_bytes / (psi_ms * 1e-3) / 1e9
+    bmin = 3 * MV * NN * 8 + cfg.n_views * NN * 4            # whole iteration (SURVEY.md 8(d))
+    bsimple = 4 * MV * NN * 8 + cfg.n_views * NN * 4
+    it_gbs = bmin / (ms_step * 1e-3) / 1e9
+    traffic, traffic_src = measured_traffic(cfg.name, info["path"], geo["wf_lag"])
+    res = {
+        "value": grp.aggregate(MV, steps, ms_total), "unit": UNIT, "steps": steps, "warmup": warmup,
+        "ms_per_step": ms_step, "iterations_per_s": 1e3 / ms_step,
+        "config": {"workload": cfg.name, "N": cfg.N, "n_views": cfg.n_views, "K": cfg.K, "L": cfg.L,
+                   "object": [cfg.obj_h, cfg.obj_w], "mode_views": MV, "path": info["path"],
+                   "parallelism": "replicas" if grp.world > 1 else "single-gpu",
+                   "l2": f"inputs larger than L2 (psi {MV * NN * 8 / 2**20:.0f} MiB streamed every step)"
+                         if MV * NN * 8 > 2 * 126 * 2**20 else "psi fits L2: latency-bound case, no flush"},
+        "roofline": {"bound": "hbm", "kernel": "psi update (S1-S6)", "achieved": achieved, "peak": peak,
+                     "unit": "GB/s", "frac": achieved / peak, "frac_of_nominal_8TBs": achieved / NOMINAL_HBM_GBS,
+                     "traffic": traffic, "traffic_source": traffic_src, "peak_source": peak_src,
+                     "bytes_per_launch": psi_bytes, "ms_per_launch": psi_ms},
+        "iteration_roofline": {"bytes_min": bmin, "bytes_simple_schedule": bsimple, "achieved_gbs": it_gbs,
+                               "frac_of_measured_hbm": it_gbs / peak, "frac_of_nominal_8TBs": it_gbs / NOMINAL_HBM_GBS},
+        "phase_ms_per_step": {k: float(v) / max(n_prof, 1) for k, v in
+                              zip(("psi_update", "object", "probe", "errors"), phase_ms)},
+        "gpu_launches": info["launches_per_iter"] * steps,
+    }
+    return plan, (I_h, P_h, O_h), res
+
+
 def run_ours(args, cfg):
     import torch
     from paper_1808_10375_b200 import dm, synth
@@ -163,90 +244,66 @@ def run_ours(args, cfg):
     grp = ReplicaGroup("nccl", torch.device("cuda", local))
     world, rank = grp.world, grp.rank
     dm.lib()
-
-    # every rank reconstructs its own data set (replicas; seed = rank)
-    pr = synth.make_problem(cfg, seed=grp.seed)
-    plan = dm.DMPlan(cfg.N, cfg.n_views, cfg.K, cfg.L, cfg.obj_h, cfg.obj_w, pr.positions,
-                     path=args.path, **({"lag": args.lag} if args.lag else {})).alloc_workspace()
-    I_h = torch.from_numpy(pr.intensities).pin_memory()
-    P_h = torch.from_numpy(pr.probe0).pin_memory()
-    O_h = torch.from_numpy(pr.object0).pin_memory()
-    Pout_h = torch.empty_like(P_h).pin_memory()
-    Oout_h = torch.empty_like(O_h).pin_memory()
-    I_d, P_d, O_d = I_h.cuda(), P_h.cuda(), O_h.cuda()
     stream = torch.cuda.current_stream()
-
-    barrier, max_over_ranks = grp.barrier, grp.max_over_ranks
-
     sampler = ClockSampler(local)
     sampler.start()
 
-    # ---- device-resident arm: inputs already in HBM, K iterations timed with CUDA events ----
-    plan.set_data(I_d, P_d, O_d)
-    plan.iterate(args.warmup)
-    plan.set_profiling(True)
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    barrier()
-    e0.record(stream)
-    plan.iterate(args.steps)
-    e1.record(stream)
-    barrier()
-    ms_total = max_over_ranks(e0.elapsed_time(e1))
-    phase_ms, n_prof = plan.phase_ms()
-    plan.set_profiling(False)
-    info = plan.info()
+    # ---- headline workload: every rank reconstructs its own data set (replicas; seed = rank) ----
+    pr = synth.make_problem(cfg, seed=grp.seed)
+    plan, (I_h, P_h, O_h), line = measure_device_arm(dm, synth, torch, grp, cfg, pr, args.steps, args.warmup,
+                                                     args.path, args.lag, stream)
 
     # ---- end-to-end arm: HOST (pinned) buffers through dm_solve_host, copies inside the timing ----
+    Pout_h = torch.empty_like(P_h).pin_memory()
+    Oout_h = torch.empty_like(O_h).pin_memory()
     e2e_steps = max(1, min(args.steps, args.e2e_steps))
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     for _ in range(2):
         plan.solve_host(I_h, P_h, O_h, 1, Pout_h, Oout_h)
-    barrier()
+    grp.barrier()
     e0.record(stream)
     for _ in range(e2e_steps):
         plan.solve_host(I_h, P_h, O_h, 1, Pout_h, Oout_h)
     e1.record(stream)
-    barrier()
-    ms_e2e = max_over_ranks(e0.elapsed_time(e1))
+    grp.barrier()
+    ms_e2e = grp.max_over_ranks(e0.elapsed_time(e1))
+    h2d = I_h.numel() * 4 + P_h.numel() * 8 + O_h.numel() * 8
+    d2h = Pout_h.numel() * 8 + Oout_h.numel() * 8
+    plan.close()
+    del plan, I_h, P_h, O_h, Pout_h, Oout_h, pr
+    torch.cuda.empty_cache()
+
+    # ---- the other single-GPU configs, same device-resident measurement (N = 1 only) ----
+    per_config = []
+    if world == 1 and not args.no_per_config:
+        for ci in args.per_config:
+            if ci == args.config:
+                continue
+            c2 = synth.CONFIGS[ci]
+            pr2 = synth.make_problem(c2, seed=grp.seed)
+            plan2, hosts, r2 = measure_device_arm(dm, synth, torch, grp, c2, pr2, args.per_config_steps, max(3, args.warmup),
+                                                  0, 0, stream)
+            plan2.close()
+            del plan2, hosts, pr2
+            torch.cuda.empty_cache()
+            per_config.append(r2)
     clocks = sampler.stop()
 
     if rank != 0:
         grp.close()
         return
 
-    MV, NN = cfg.mode_views, cfg.N * cfg.N
-    ms_step = ms_total / args.steps
-    value = grp.aggregate(MV, args.steps, ms_total)
-    peak, peak_src = measured_peaks()
-    psi_bytes = MV * NN * 16 + cfg.n_views * NN * 4          # psi read + write + sqrt(I) read
-    psi_ms = phase_ms[0] / max(n_prof, 1)
-    achieved = psi_bytes / (psi_ms * 1e-3) / 1e9
-    bmin = 3 * MV * NN * 8 + cfg.n_views * NN * 4            # whole iteration
-    h2d = I_h.numel() * 4 + P_h.numel() * 8 + O_h.numel() * 8
-    d2h = Pout_h.numel() * 8 + Oout_h.numel() * 8
-    line = {
-        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
-        "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak",
-        "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-        "iterations_per_s": 1e3 / ms_step,
-        "config": {"workload": cfg.name, "N": cfg.N, "n_views": cfg.n_views, "K": cfg.K, "L": cfg.L,
-                   "object": [cfg.obj_h, cfg.obj_w], "mode_views": MV, "path": info["path"],
-                   "parallelism": "replicas" if world > 1 else "single-gpu",
-                   "l2": f"inputs larger than L2 (psi {MV * NN * 8 / 2**20:.0f} MiB streamed every step)"
-                         if MV * NN * 8 > 2 * 126 * 2**20 else "psi fits L2: latency-bound case, no flush"},
-        "roofline": {"bound": "hbm", "kernel": "psi update (S1-S6)", "achieved": achieved, "peak": peak,
-                     "unit": "GB/s", "frac": achieved / peak, "traffic": measured_traffic(cfg.name, info["path"]),
-                     "peak_source": peak_src,
-                     "bytes_per_launch": psi_bytes, "ms_per_launch": psi_ms},
-        "iteration_roofline": {"bytes_min": bmin, "achieved_gbs": bmin / (ms_step * 1e-3) / 1e9,
-                               "frac_of_measured_hbm": bmin / (ms_step * 1e-3) / 1e9 / peak},
-        "phase_ms_per_step": {k: float(v) / max(n_prof, 1) for k, v in
-                              zip(("psi_update", "object", "probe", "errors"), phase_ms)},
-        "e2e": {"value": grp.aggregate(MV, e2e_steps, ms_e2e), "unit": UNIT, "steps": e2e_steps,
-                "ms_per_step": ms_e2e / e2e_steps, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
-                "call": "dm_solve_host(n_iter=1): H2D intensities+P0+O0 (pinned), set_data, 1 iteration, D2H P+O"},
-        "gpu_launches": info["launches_per_iter"] * args.steps,
-        "clocks": clocks,
-    }
+    head = {"metric": METRIC, "value": line.pop("value"), "unit": line.pop("unit"), "n_gpus": world,
+            "steps": line.pop("steps"), "warmup": line.pop("warmup"), "ms_per_step": line.pop("ms_per_step"),
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic"}
+    head.update(line)
+    head["e2e"] = {"value": grp.aggregate(cfg.mode_views, e2e_steps, ms_e2e), "unit": UNIT, "steps": e2e_steps,
+                   "ms_per_step": ms_e2e / e2e_steps, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+                   "call": "dm_solve_host(n_iter=1): H2D intensities+P0+O0 (pinned), set_data, 1 iteration, D2H P+O"}
+    head["clocks"] = clocks
+    if per_config:
+        head["per_config"] = per_config
+    line = head
     if world == 1 and not args.no_cpu_baseline:
         v, ms, cores, sample = time_oracle(cfg, 1, 1, args.ref_mode_views)
         line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample,
@@ -262,17 +319,28 @@ def run_ours(args, cfg):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=100)
+    ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=5)
-    ap.add_argument("--config", type=int, default=1, help="BASELINE.json config index (default 1)")
+    ap.add_argument("--config", type=int, default=3,
+                    help="BASELINE.json config index of the headline workload (default 3: the largest single-GPU config)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--path", type=int, default=0, help="0 auto, 1 staged, 2 fused")
+    ap.add_argument("--path", type=int, default=0,
+                    help="psi-update path of the headline workload: 0 auto, 1 staged, 2 fused (N <= 128), "
+                         "3 register-resident (N = 128), 4 view-pipelined warp-FFT, 5 half-frame clusters (N = 128)")
     ap.add_argument("--lag", type=int, default=0, help="path 4: phase lag in views (0 = derived)")
-    ap.add_argument("--e2e-steps", type=int, default=20)
+    ap.add_argument("--e2e-steps", type=int, default=5)
+    ap.add_argument("--per-config", type=int, nargs="*", default=[1, 2, 4],
+                    help="other configs measured in the same run (device-resident arm only), reported under per_config")
+    ap.add_argument("--per-config-steps", type=int, default=10)
+    ap.add_argument("--no-per-config", action="store_true")
+    ap.add_argument("--print-csrc-digest", action="store_true", help="print the digest profiles/traffic.json is keyed by")
     ap.add_argument("--ref-mode-views", type=int, default=4096,
                     help="size of the bounded oracle sample (mode-views per iteration)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
+    if args.print_csrc_digest:
+        print(csrc_digest())
+        return
     from paper_1808_10375_b200 import synth
     cfg = synth.CONFIGS[args.config]
     if args.impl == "reference":

@@ -87,8 +87,10 @@ dm_status dm_plan_create(dm_plan **out, int N, int n_views, int K, int L, int ob
 dm_status dm_plan_set_param(dm_plan *plan, dm_param which, double value);
 
 /* Bytes of device workspace the plan needs (psi, sqrt(I), P/O double buffers, tables,
- * partial sums, error table, L2 scratch of the staged path).                          */
-dm_status dm_plan_workspace_bytes(const dm_plan *plan, size_t *bytes);
+ * partial sums, error table, L2 scratch of the staged path).  Asks the current CUDA
+ * device for its SM count (the reduction geometry and the persistent grids follow it;
+ * without a device the B200's 148 is assumed).                                        */
+dm_status dm_plan_workspace_bytes(dm_plan *plan, size_t *bytes);
 
 /* Lend the workspace: DEV pointer, 256-byte aligned, >= dm_plan_workspace_bytes.  Borrowed
  * until dm_plan_destroy; contents are the library's.                                   */
@@ -157,6 +159,19 @@ dm_status dm_solve_host(dm_plan *plan, const float *intensities_host, const floa
  * after dm_set_data);
  * and how many kernels one iteration launches (the bench's gpu_launches claim).           */
 dm_status dm_plan_info(const dm_plan *plan, int *path, int *launches_per_iter);
+
+/* Launch geometry the kernels of this plan run with (test / measurement aid; HOST output, no
+ * CUDA call).  The parity tests assert through it that they reach the loop shapes of the
+ * full-size launches.  Writes min(n_out, DM_GEOMETRY_FIELDS) int32 values:
+ *   [0] psi-update path (as dm_plan_info)      [1] SM count the grids were sized for
+ *   [2] probe update (eq. (5)): CTAs along the view axis   [3] views summed by each of them
+ *   [4] object update (eq. (6)): longest coverage list     [5] list entries per batch
+ *   [6] paths 3, 5: persistent CTAs   [7] CTAs per view   [8] most views one of their groups takes
+ *   [9] path 4: scratch ring slots    [10] phase lag (views)   [11] persistent CTAs   [12] warps per CTA
+ *   [13] path 3: 1 = the CTAs of a view meet at a software barrier in L2, 0 = hardware cluster
+ * [6]-[8], [11] and [13] are valid after dm_set_data (they come from occupancy queries).          */
+#define DM_GEOMETRY_FIELDS 14
+dm_status dm_plan_geometry(const dm_plan *plan, int32_t *out_host, int n_out);
 
 /* Per-phase device timing (measurement aid of bench.py; off by default).  When on, dm_iterate
  * records CUDA events on `stream` around the four phases of every iteration (psi update S1-S6,

@@ -1,5 +1,6 @@
 // dm_api.cu -- the C ABI of include/dm.h: host plan (integer tables, workspace carving),
 // launch orchestration of one DM iteration, getters.  No torch types, no exceptions.
+#include <algorithm>
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
@@ -19,7 +20,6 @@ constexpr int ERR_ROWS_CAP = 16384;
 constexpr size_t SCRATCH_TARGET = 48u << 20;     // staged path: spectra of one chunk stay in L2
 constexpr int COLS_SW = 8;                        // staged path: spectrum columns per CTA
 constexpr int PROF_MAX_ITERS = 4096;
-constexpr int REG_MAX_CTAS = 160;                 // path 3: upper bound on resident CTAs (B200: 148 SMs)
 
 thread_local std::string g_create_error;
 
@@ -39,7 +39,8 @@ struct dm_plan {
     int path_req, path;                  // requested / chosen (1 staged, 2 fused, 3 register-resident)
     int reg_grid;                        // path 3: number of persistent CTAs (multiple of M)
     bool reg_sw;                         // path 3: software group barrier instead of a hardware cluster
-    int *reg_gbar;                       // path 3: [REG_MAX_CTAS] group barrier counters
+    int *reg_gbar;                       // path 3: [reg_cap] group barrier counters
+    int reg_cap;                         // paths 3, 5: upper bound on resident CTAs (2 per SM)
     // path 4 (dm_warpfft.cuh): ring slots, phase lag (views), tasks per view and phase, persistent CTAs
     int wf_S, wf_D, wf_nA, wf_nB, wf_nC, wf_grid, wf_nw;
     int wf_lag_req;                      // 0 = derive the lag from the task counts
@@ -79,6 +80,8 @@ struct dm_plan {
     double2 *psi64, *scr64, *P64[2], *O64[2], *tw64;
     double *amp64, *den64, *alphas64, *partF64, *partS64, *partP64, *partO64;
     int tables_path;                     // path whose tables / twiddles are on the device (0: none)
+    int sms;                             // SM count of the device (148 until a CUDA call could ask)
+    int max_list;                        // longest coverage list (object_gather_kernel batches it by OBJ_NT)
     mutable std::string err;
 };
 
@@ -121,6 +124,8 @@ void build_tables(dm_plan *p)
     }
     for (int t = 0; t < nt; ++t) cnt[t + 1] += cnt[t];
     p->tile_ptr = cnt;
+    p->max_list = 0;
+    for (int t = 0; t < nt; ++t) p->max_list = std::max(p->max_list, cnt[t + 1] - cnt[t]);
     p->tile_views.assign((size_t)cnt[nt], 0);
     std::vector<int32_t> fill(cnt.begin(), cnt.end() - 1);
     for (int j = 0; j < p->n_views; ++j) {     // j ascending -> every list ascending
@@ -146,12 +151,13 @@ void plan_geometry(dm_plan *p)
 {
     const size_t NN = (size_t)p->N * p->N;
     p->prb_blocks = (int)((NN / 2 + PRB_NT - 1) / PRB_NT);
-    int chunks = (148 * 16 + p->prb_blocks - 1) / p->prb_blocks;        // ~16 CTAs per SM in flight
+    int chunks = (p->sms * 16 + p->prb_blocks - 1) / p->prb_blocks;     // ~16 CTAs per SM in flight
     if (chunks > p->n_views) chunks = p->n_views;
     if (chunks < 1) chunks = 1;
     p->prb_chunk_len = (p->n_views + chunks - 1) / chunks;
     p->prb_chunks = (p->n_views + p->prb_chunk_len - 1) / p->prb_chunk_len;
     p->fin_blocks = (int)((NN + 255) / 256);
+    p->reg_cap = 2 * p->sms;
     const size_t per_view = (size_t)p->M * NN * sizeof(float2);
     size_t cv = SCRATCH_TARGET / per_view;
     if (cv < 1) cv = 1;
@@ -167,7 +173,7 @@ void plan_geometry(dm_plan *p)
     const int T = p->wf_nA + p->wf_nB + p->wf_nC;
     // lag: a phase starts on a view once ~1.6 x (resident CTAs) tasks have been queued behind its inputs
     // (measured on B200 at the end of round 1: c3 is fastest at 3-4 views, c4 at 2; a longer lag only pushes psi out of L2)
-    const int resident = 148 * (16 / p->wf_nw);
+    const int resident = p->sms * (16 / p->wf_nw);
     int D = p->wf_lag_req > 0 ? p->wf_lag_req : (int)((1.6 * resident + T - 1) / T);
     if (D < 1) D = 1;
     p->wf_D = D;
@@ -200,7 +206,7 @@ size_t carve(dm_plan *p, unsigned char *base)
     p->den_tmp = (float *)take((HW > NN ? HW : NN) * sizeof(float));
     p->alphas = (float *)take(2 * sizeof(float));
     size_t nA = (size_t)p->nA * 2 > MV * 4 ? (size_t)p->nA * 2 : MV * 4;
-    if (nA < (size_t)REG_MAX_CTAS * 4) nA = (size_t)REG_MAX_CTAS * 4;
+    if (nA < (size_t)p->reg_cap * 4) nA = (size_t)p->reg_cap * 4;
     if (nA < (size_t)p->n_views * p->wf_nB * 2) nA = (size_t)p->n_views * p->wf_nB * 2;
     size_t nB = (size_t)p->nB * 2;
     if (nB < (size_t)p->n_views * p->wf_nC * 2) nB = (size_t)p->n_views * p->wf_nC * 2;
@@ -214,8 +220,8 @@ size_t carve(dm_plan *p, unsigned char *base)
     p->spec_d = (int *)take(NN * sizeof(int));
     p->wy_d = (float2 *)take(128 * sizeof(float2));
     p->wx_d = (float2 *)take(128 * sizeof(float2));
-    p->sbuf = (float4 *)take(p->N == 128 ? (size_t)2 * REG_MAX_CTAS * 8 * dmreg::RNT * sizeof(float4) : 0);
-    p->reg_gbar = (int *)take(REG_MAX_CTAS * sizeof(int));
+    p->sbuf = (float4 *)take(p->N == 128 ? (size_t)2 * p->reg_cap * 8 * dmreg::RNT * sizeof(float4) : 0);
+    p->reg_gbar = (int *)take((size_t)p->reg_cap * sizeof(int));
     p->tw_d = (float2 *)take(p->N * sizeof(float2));
     p->mode_pow = (double *)take((size_t)(p->K + p->L) * sizeof(double));
     p->errors = (double *)take((size_t)ERR_ROWS_CAP * (2 + p->K + p->L) * sizeof(double));
@@ -257,13 +263,15 @@ PsiArgs psi_args(const dm_plan *p)
     return a;
 }
 
-template <int N, int NT> dm_status launch_fused(dm_plan *plan, cudaStream_t st)
+// Every launch_* below takes `prepare`: true = called once per plan from dm_set_data on the plan's device to
+// opt the kernel in to its dynamic shared memory (a per-device function attribute) and to size the persistent
+// grids from occupancy queries; nothing is launched then.
+template <int N, int NT> dm_status launch_fused(dm_plan *plan, cudaStream_t st, bool prepare)
 {
     const size_t smem = (size_t)N * N * (sizeof(float2) + sizeof(float)) + N * sizeof(float2);
-    static bool attr_done = false;
-    if (!attr_done) {
+    if (prepare) {
         CU(cudaFuncSetAttribute(fused_frame_kernel<N, NT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        attr_done = true;
+        return DM_OK;
     }
     PsiArgs a = psi_args(plan);
     cudaLaunchConfig_t cfg;
@@ -283,14 +291,15 @@ template <int N, int NT> dm_status launch_fused(dm_plan *plan, cudaStream_t st)
     return DM_OK;
 }
 
-template <int N> dm_status launch_staged(dm_plan *plan, cudaStream_t st)
+template <int N> dm_status launch_staged(dm_plan *plan, cudaStream_t st, bool prepare)
 {
     constexpr int ROWS = 4096 / N, NT = 256, SW = COLS_SW;
     const size_t smem = (size_t)plan->M * N * SW * sizeof(float2);
-    static bool attr_done = false;
-    if (!attr_done) {
+    if (prepare) {
+        if (smem > 200 * 1024)
+            return fail(plan, DM_ERR_UNSUPPORTED, "staged path: %d modes of N = %d need %zu bytes of shared memory per CTA", plan->M, N, smem);
         CU(cudaFuncSetAttribute(cols_mod_kernel<N, SW, NT>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
-        attr_done = true;
+        return DM_OK;
     }
     PsiArgs a = psi_args(plan);
     for (int v0 = 0; v0 < plan->n_views; v0 += plan->chunk_views) {
@@ -310,11 +319,7 @@ template <int N> dm_status launch_staged(dm_plan *plan, cudaStream_t st)
 template <int MT> dm_status launch_regfft_t(dm_plan *plan, cudaStream_t st, bool query_only)
 {
     auto kern = dmreg::regfft128_kernel<MT>;
-    static bool attr_done = false;
-    if (!attr_done) {
-        CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, dmreg::REG_SMEM_V1));
-        attr_done = true;
-    }
+    if (query_only) CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, dmreg::REG_SMEM_V1));
     cudaLaunchConfig_t cfg;
     memset(&cfg, 0, sizeof cfg);
     cfg.blockDim = dim3(dmreg::RNT);
@@ -345,7 +350,7 @@ template <int MT> dm_status launch_regfft_t(dm_plan *plan, cudaStream_t st, bool
         }
         if (ncl < 1) return fail(plan, DM_ERR_CUDA, "register-resident kernel: no cluster of %d CTAs fits", plan->M);
         if (ncl > plan->n_views) ncl = plan->n_views;
-        if (ncl * plan->M > REG_MAX_CTAS) ncl = REG_MAX_CTAS / plan->M;
+        if (ncl * plan->M > plan->reg_cap) ncl = plan->reg_cap / plan->M;
         plan->reg_grid = ncl * plan->M;
         return DM_OK;
     }
@@ -359,7 +364,7 @@ template <int MT> dm_status launch_regfft_t(dm_plan *plan, cudaStream_t st, bool
     cfg.gridDim = dim3((unsigned)plan->reg_grid);
     if (plan->reg_sw) {
         a.gbar = plan->reg_gbar;
-        CU(cudaMemsetAsync(plan->reg_gbar, 0, REG_MAX_CTAS * sizeof(int), st));
+        CU(cudaMemsetAsync(plan->reg_gbar, 0, (size_t)plan->reg_cap * sizeof(int), st));
         at[0].id = cudaLaunchAttributeCooperative;      // all CTAs resident: they wait on one another
         at[0].val.cooperative = 1;
         cfg.numAttrs = 1;
@@ -385,12 +390,9 @@ template <int N> dm_status launch_wf_t(dm_plan *plan, cudaStream_t st, bool quer
     auto kern = dmwf::wf_dataflow_kernel<N>;
     const int nt = 32 * plan->wf_nw;
     const int smem = plan->wf_nw * dmwf::WF_XBUF + (N / 32) * 32 * (int)sizeof(float2) + (plan->wf_nw / plan->M) * 4096;
-    static bool attr_done = false;
-    if (!attr_done) {
+    if (query_only)
         CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                 dmwf::WF_MAXW * dmwf::WF_XBUF + (N / 32) * 32 * (int)sizeof(float2) + dmwf::WF_MAXW * 4096));
-        attr_done = true;
-    }
     if (query_only) {
         int dev = 0, sms = 0, per = 0;
         CU(cudaGetDevice(&dev));
@@ -427,19 +429,19 @@ dm_status launch_wf(dm_plan *plan, cudaStream_t st, bool query_only)
     }
 }
 
-dm_status launch_psi_update(dm_plan *plan, cudaStream_t st)
+dm_status launch_psi_update(dm_plan *plan, cudaStream_t st, bool prepare = false)
 {
-    if (plan->path == 4) return launch_wf(plan, st, false);
-    if (plan->path == 3) return launch_regfft(plan, st, false);
+    if (plan->path == 4) return launch_wf(plan, st, prepare);
+    if (plan->path == 3) return launch_regfft(plan, st, prepare);
     if (plan->path == 2) {
-        if (plan->N == 64) return launch_fused<64, 256>(plan, st);
-        return launch_fused<128, 512>(plan, st);
+        if (plan->N == 64) return launch_fused<64, 256>(plan, st, prepare);
+        return launch_fused<128, 512>(plan, st, prepare);
     }
     switch (plan->N) {
-    case 64: return launch_staged<64>(plan, st);
-    case 128: return launch_staged<128>(plan, st);
-    case 256: return launch_staged<256>(plan, st);
-    default: return launch_staged<512>(plan, st);
+    case 64: return launch_staged<64>(plan, st, prepare);
+    case 128: return launch_staged<128>(plan, st, prepare);
+    case 256: return launch_staged<256>(plan, st, prepare);
+    default: return launch_staged<512>(plan, st, prepare);
     }
 }
 
@@ -500,6 +502,21 @@ dm_status launch_probe(dm_plan *plan, cudaStream_t st, const float2 *O, const fl
     return DM_OK;
 }
 
+// The grids and the reduction geometry follow the SM count of the current device; without a device
+// (CPU-only callers of the host tables) the B200's 148 stays.  Re-measures the workspace.
+void adopt_device(dm_plan *p)
+{
+    int dev = 0, sms = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || sms < 1) {
+        cudaGetLastError();
+        return;
+    }
+    if (sms == p->sms) return;
+    p->sms = sms;
+    plan_geometry(p);
+    p->need_bytes = carve(p, nullptr);
+}
+
 dm_status check_ready(const dm_plan *plan, bool need_data)
 {
     if (!plan) return DM_ERR_INVALID_ARG;
@@ -541,6 +558,7 @@ dm_status dm_plan_create(dm_plan **out, int N, int n_views, int K, int L, int ob
     p->ws = nullptr; p->ws_bytes = 0;
     p->curP = p->curO = 0; p->has_data = false; p->rows = 0;
     p->profiling = false; p->ev_iters = 0; p->copy_ready = false; p->tables_path = 0; p->precision = 0;
+    p->sms = 148;
     build_tables(p);
     plan_geometry(p);
     p->need_bytes = carve(p, nullptr);
@@ -577,9 +595,10 @@ dm_status dm_plan_set_param(dm_plan *plan, dm_param which, double v)
     return fail(plan, DM_ERR_INVALID_ARG, "parameter %d: value %g out of range", (int)which, v);
 }
 
-dm_status dm_plan_workspace_bytes(const dm_plan *plan, size_t *bytes)
+dm_status dm_plan_workspace_bytes(dm_plan *plan, size_t *bytes)
 {
     if (!plan || !bytes) return DM_ERR_INVALID_ARG;
+    if (!plan->ws) adopt_device(plan);
     *bytes = plan->need_bytes;
     return DM_OK;
 }
@@ -589,6 +608,7 @@ dm_status dm_plan_set_workspace(dm_plan *plan, void *dev, size_t bytes)
     if (!plan) return DM_ERR_INVALID_ARG;
     if (!dev) return fail(plan, DM_ERR_INVALID_ARG, "workspace pointer is NULL");
     if ((uintptr_t)dev % ALIGN) return fail(plan, DM_ERR_WORKSPACE, "workspace must be 256-byte aligned");
+    adopt_device(plan);
     if (bytes < plan->need_bytes)
         return fail(plan, DM_ERR_WORKSPACE, "workspace of %zu bytes < %zu needed", bytes, plan->need_bytes);
     plan->ws = dev;
@@ -602,7 +622,7 @@ dm_status dm_plan_set_workspace(dm_plan *plan, void *dev, size_t bytes)
 } // extern "C"
 
 namespace {
-constexpr int CONV_GRID = 148 * 8;
+constexpr int CONV_GRID = 148 * 8;                 // grid-stride conversion kernels: any grid is correct
 
 dm64::Args args64(const dm_plan *p)
 {
@@ -744,8 +764,6 @@ dm_status set_data_impl(dm_plan *plan, const float *intensities, const float *pr
         CU(cudaMemcpyAsync(plan->wy_d, wy.data(), 256 * sizeof(float), cudaMemcpyHostToDevice, st));
         CU(cudaMemcpyAsync(plan->wx_d, wx.data(), 256 * sizeof(float), cudaMemcpyHostToDevice, st));
         CU(cudaStreamSynchronize(st));          // wy / wx are stack-owned host buffers
-        dm_status qs = launch_regfft(plan, st, true);
-        if (qs != DM_OK) return qs;
     } else if (path == 4) {
         const int N = plan->N, RX = N / 32, G = 32 / RX;
         for (int cg = 0; cg < N / G; ++cg)
@@ -769,8 +787,6 @@ dm_status set_data_impl(dm_plan *plan, const float *intensities, const float *pr
             }
         CU(cudaMemcpyAsync(plan->wf_tw_d, tw.data(), tw.size() * sizeof(float), cudaMemcpyHostToDevice, st));
         CU(cudaStreamSynchronize(st));          // tw is a stack-owned host buffer
-        dm_status qs = launch_wf(plan, st, true);
-        if (qs != DM_OK) return qs;
     } else {
         for (int py = 0; py < plan->N; ++py)
             for (int px = 0; px < plan->N; ++px) plan->spec[(size_t)py * plan->N + px] = plan->rev[py] * plan->N + plan->rev[px];
@@ -782,6 +798,10 @@ dm_status set_data_impl(dm_plan *plan, const float *intensities, const float *pr
     CU(cudaMemcpyAsync(plan->spec_d, plan->spec.data(), plan->spec.size() * sizeof(int32_t), cudaMemcpyHostToDevice, st));
     CU(cudaMemcpyAsync(plan->tw_d, plan->tw.data(), plan->tw.size() * sizeof(float), cudaMemcpyHostToDevice, st));
     CU(cudaStreamSynchronize(st));              // pageable host sources
+    if (path != 64) {
+        dm_status qs = launch_psi_update(plan, st, true);      // function attributes + occupancy-sized grids
+        if (qs != DM_OK) return qs;
+    }
     plan->tables_path = path;
     }
     if (plan->precision == 1) {
@@ -797,7 +817,7 @@ dm_status set_data_impl(dm_plan *plan, const float *intensities, const float *pr
     CU(cudaMemcpyAsync(plan->Obuf[0], object0, plan->L * HW * sizeof(float2), cudaMemcpyDeviceToDevice, st));
     CU(cudaMemsetAsync(plan->alphas, 0, 2 * sizeof(float), st));
     const size_t total = (size_t)plan->n_views * NN;
-    if (n_chunks <= 0) amp_permute_kernel<<<148 * 8, 256, 0, st>>>(plan->N, intensities, plan->spec_d, plan->amp, total);
+    if (n_chunks <= 0) amp_permute_kernel<<<plan->sms * 8, 256, 0, st>>>(plan->N, intensities, plan->spec_d, plan->amp, total);
     psi_init_kernel<<<dim3((unsigned)((NN + 1023) / 1024), (unsigned)(plan->n_views * plan->M)), 256, 0, st>>>(
         plan->N, plan->K, plan->L, plan->H, plan->W, plan->pos_d, plan->Pbuf[0], plan->Obuf[0], plan->psi);
     CU(cudaGetLastError());
@@ -814,7 +834,7 @@ dm_status set_data_impl(dm_plan *plan, const float *intensities, const float *pr
         const int v0 = (int)((long long)plan->n_views * c / n_chunks), v1 = (int)((long long)plan->n_views * (c + 1) / n_chunks);
         if (v1 == v0) continue;
         CU(cudaStreamWaitEvent(st, chunk_ev[c], 0));
-        amp_permute_kernel<<<148 * 8, 256, 0, st>>>(plan->N, intensities + (size_t)v0 * NN, plan->spec_d,
+        amp_permute_kernel<<<plan->sms * 8, 256, 0, st>>>(plan->N, intensities + (size_t)v0 * NN, plan->spec_d,
                                                     plan->amp + (size_t)v0 * NN, (size_t)(v1 - v0) * NN);
     }
     CU(cudaGetLastError());
@@ -1118,6 +1138,22 @@ dm_status dm_plan_info(const dm_plan *plan, int *path, int *launches_per_iter)
         const int chunks = (plan->n_views + plan->chunk_views - 1) / plan->chunk_views;
         *launches_per_iter = p == 64 ? 8 : (p >= 2 ? 1 : 3 * chunks) + 4;
     }
+    return DM_OK;
+}
+
+dm_status dm_plan_geometry(const dm_plan *plan, int32_t *out_host, int n_out)
+{
+    if (!plan || !out_host || n_out < 0) return DM_ERR_INVALID_ARG;
+    int path = 0;
+    dm_plan_info(plan, &path, nullptr);
+    const bool reg = path == 3 || path == 5;
+    const int per_view = path == 5 ? 2 * plan->M : plan->M;
+    const int clusters = reg && plan->reg_grid > 0 ? plan->reg_grid / per_view : 0;
+    const int32_t g[DM_GEOMETRY_FIELDS] = {
+        path, plan->sms, plan->prb_chunks, plan->prb_chunk_len, plan->max_list, OBJ_NT,
+        reg ? plan->reg_grid : 0, reg ? per_view : 0, clusters ? (plan->n_views + clusters - 1) / clusters : 0,
+        plan->wf_S, plan->wf_D, path == 4 ? plan->wf_grid : 0, plan->wf_nw, reg && plan->reg_sw ? 1 : 0};
+    for (int i = 0; i < n_out && i < DM_GEOMETRY_FIELDS; ++i) out_host[i] = g[i];
     return DM_OK;
 }
 

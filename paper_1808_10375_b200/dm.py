@@ -24,7 +24,7 @@ SYMBOLS = (
     "dm_plan_create", "dm_plan_set_param", "dm_plan_workspace_bytes", "dm_plan_set_workspace",
     "dm_set_data", "dm_iterate", "dm_get_probe", "dm_get_object", "dm_get_psi", "dm_get_errors",
     "dm_set_state", "dm_get_window_table", "dm_get_coverage", "dm_get_alphas", "dm_get_mode_power", "dm_solve_host",
-    "dm_plan_info", "dm_plan_set_profiling", "dm_get_phase_ms", "dm_host_fft2", "dm_host_fft2_path", "dm_status_string", "dm_last_error", "dm_plan_destroy",
+    "dm_plan_info", "dm_plan_geometry", "dm_plan_set_profiling", "dm_get_phase_ms", "dm_host_fft2", "dm_host_fft2_path", "dm_status_string", "dm_last_error", "dm_plan_destroy",
 )
 
 _vp, _int, _dbl = C.c_void_p, C.c_int, C.c_double
@@ -62,6 +62,7 @@ def lib() -> C.CDLL:
         L.dm_get_mode_power.argtypes = [_vp, _vp]
         L.dm_solve_host.argtypes = [_vp, _vp, _vp, _vp, _int, _vp, _vp, _vp]
         L.dm_plan_info.argtypes = [_vp, C.POINTER(_int), C.POINTER(_int)]
+        L.dm_plan_geometry.argtypes = [_vp, _vp, _int]
         L.dm_plan_set_profiling.argtypes = [_vp, _int]
         L.dm_get_phase_ms.argtypes = [_vp, _vp, C.POINTER(_int)]
         L.dm_host_fft2.argtypes = [_int, _vp, _vp, _int]
@@ -214,6 +215,15 @@ class DMPlan:
         p, n = _int(), _int()
         self._check(self._lib.dm_plan_info(self._h, C.byref(p), C.byref(n)))
         return {"path": p.value, "launches_per_iter": n.value}
+
+    GEOMETRY = ("path", "sms", "prb_chunks", "prb_chunk_len", "obj_max_list", "obj_batch", "reg_grid",
+                "reg_ctas_per_view", "reg_views_per_group", "wf_slots", "wf_lag", "wf_grid", "wf_warps", "reg_sw_barrier")
+
+    def geometry(self):
+        """dm_plan_geometry: the launch geometry as a dict (valid after set_data)."""
+        out = np.zeros(len(self.GEOMETRY), np.int32)
+        self._check(self._lib.dm_plan_geometry(self._h, _np_ptr(out), len(out)))
+        return dict(zip(self.GEOMETRY, (int(v) for v in out)))
 
     def set_profiling(self, on=True):
         self._check(self._lib.dm_plan_set_profiling(self._h, int(bool(on))))

@@ -39,12 +39,55 @@ def make_pair(dm, pr, **params):
     return g, o
 
 
-def compare_state(g, o, tol, what=""):
-    r = {"psi": synth.rel_l2(g.psi().cpu().numpy(), o.psi()),
-         "P": synth.rel_l2(g.probe().cpu().numpy(), o.probe()),
-         "O": synth.rel_l2(g.object().cpu().numpy(), o.object())}
-    for k, v in r.items():
-        assert v <= tol, f"{what} {k}: rel L2 {v:.3e} > {tol:g}  ({r})"
+MAXABS_FACTOR = 10.0      # max |delta| <= 10 tol * max |ref|: no isolated wrong element hides under the norm
+
+
+def _cmp(a, b, block=64):
+    """(relative L2, max |a - b| / max |b|) of two equally shaped arrays, computed in blocks along axis 0
+    so that the full-size states (GiB) need no full-size temporaries."""
+    num = den = 0.0
+    dmax = bmax = 0.0
+    for i in range(0, a.shape[0], block):
+        x = np.asarray(a[i:i + block]).astype(np.complex128)
+        y = np.asarray(b[i:i + block]).astype(np.complex128)
+        d = np.abs(x - y)
+        num += float((d * d).sum())
+        den += float((np.abs(y) ** 2).sum())
+        dmax = max(dmax, float(d.max()))
+        bmax = max(bmax, float(np.abs(y).max()))
+    return (num / den) ** 0.5 if den > 0 else num ** 0.5, dmax / bmax if bmax > 0 else dmax
+
+
+def den_object(pos, P, H, W):
+    """sum_{j covering r} sum_k |P_k|^2 (the denominator of eq. (6)) by plain numpy window adds: only used to
+    pick the well-lit object pixels a comparison is restricted to (comparison utility)."""
+    w = (np.abs(np.asarray(P).astype(np.complex128)) ** 2).sum(axis=0)
+    N = w.shape[-1]
+    den = np.zeros((H, W))
+    for y0, x0 in np.asarray(pos):
+        den[y0:y0 + N, x0:x0 + N] += w
+    return den
+
+
+def compare_state(g, o, tol, what="", lit_pos=None):
+    """psi, P, O of the CUDA path against the oracle: relative L2 <= tol (north_star's measure) AND the largest
+    element-wise deviation <= MAXABS_FACTOR * tol * max |ref| (an isolated wrong pixel cannot hide in the norm).
+    With lit_pos (the scan positions) O is also compared on the well-lit pixels alone (den_O >= 10 % of its
+    maximum), where never-illuminated border pixels, which just keep O_old, do not dilute the ratio."""
+    Og, Oo = g.object().cpu().numpy(), o.object()
+    pairs = {"psi": (g.psi().cpu().numpy(), o.psi()), "P": (g.probe().cpu().numpy(), o.probe()), "O": (Og, Oo)}
+    r = {}
+    for k, (a, b) in pairs.items():
+        r[k], mx = _cmp(a, b)
+        assert r[k] <= tol, f"{what} {k}: rel L2 {r[k]:.3e} > {tol:g}  ({r})"
+        assert mx <= MAXABS_FACTOR * tol, f"{what} {k}: max |delta| / max |ref| = {mx:.3e} > {MAXABS_FACTOR * tol:g}"
+        r[k + "_max"] = mx
+    del pairs
+    if lit_pos is not None:
+        den = den_object(lit_pos, o.probe(), o.H, o.W)
+        lit = den >= 0.1 * den.max()
+        r["O_lit"] = synth.rel_l2(Og[:, lit], Oo[:, lit])
+        assert r["O_lit"] <= tol, f"{what} O on the {lit.mean():.0%} well-lit pixels: rel L2 {r['O_lit']:.3e} > {tol:g}"
     return r
 
 
@@ -83,7 +126,7 @@ def test_one_iteration_parity(dm, cfg_i, ny, nx, path):
     g, o = forced_pair(dm, pr, 1, path=path)
     g.iterate(1)
     o.iterate(1)
-    r = compare_state(g, o, ONE_STEP_TOL, f"cfg{cfg_i} path{path} one step from t=1")
+    r = compare_state(g, o, ONE_STEP_TOL, f"cfg{cfg_i} path{path} one step from t=1", lit_pos=pr.positions)
     print(f"cfg{cfg_i} path{path}: one-step rel L2 {r}")
     eg, eo = g.errors()[-1], o.errors()[-1]
     assert eg.shape == eo.shape == (2 + pr.cfg.K + pr.cfg.L,)
@@ -97,19 +140,31 @@ def test_first_iteration_from_initial_state(dm, cfg_i, ny, nx):
     rounding floor (~1e-7 * max|F|) at bins where the data still hold counts, and eq. (4) keeps
     the *computed phase* there -- FP32 arithmetic decides it (DESIGN.md "FP32 and the first
     iteration").  Any FP32 FFT shows it: the oracle's own float build is the yardstick.  The GPU
-    must be within max(1e-5, 2 x yardstick) and the error rows within 1e-3."""
+    must be within max(1e-5, 1.5 x yardstick), the error rows within 1e-3 -- and, so that a kernel
+    defect of the size of that FP32 floor cannot hide under the yardstick, psi_new is also compared in
+    the spectrum domain on the bins where FP32 IS well conditioned (|FFT(P0 O0)| > 1e-4 of its
+    maximum, per mode frame) at the plain 1e-5 bar (the oracle's own FP32 build measures 1e-6 there)."""
     pr = synth.make_problem(synth.CONFIGS[cfg_i].scaled(ny, nx))
     c = pr.cfg
     g, o = make_pair(dm, pr)
     o32 = oracle.OracleDM(c.N, c.K, c.L, c.obj_h, c.obj_w, pr.positions, real="f32")
     o32.set_data(pr.intensities, pr.probe0, pr.object0)
+    F0 = np.abs(np.fft.fft2(o.psi()))
+    well = F0 > 1e-4 * F0.max(axis=(-2, -1), keepdims=True)
+    del F0
     g.iterate(1); o.iterate(1); o32.iterate(1)
     for name, a, b, y in (("psi", g.psi().cpu().numpy(), o.psi(), o32.psi()),
                           ("P", g.probe().cpu().numpy(), o.probe(), o32.probe()),
                           ("O", g.object().cpu().numpy(), o.object(), o32.object())):
         r, yard = synth.rel_l2(a, b), synth.rel_l2(y, b)
         print(f"cfg{cfg_i} first iteration {name}: GPU vs FP64 {r:.3e}; oracle FP32 vs FP64 {yard:.3e}")
-        assert r <= max(ONE_STEP_TOL, 2 * yard), f"{name}: {r:.3e} vs yardstick {yard:.3e}"
+        assert r <= max(ONE_STEP_TOL, 1.5 * yard), f"{name}: {r:.3e} vs yardstick {yard:.3e}"
+    Fo = np.fft.fft2(o.psi())
+    Fd = np.fft.fft2(g.psi().cpu().numpy().astype(np.complex128) - o.psi())
+    rw = float(np.linalg.norm(Fd[well]) / np.linalg.norm(Fo[well]))
+    print(f"cfg{cfg_i} first iteration, spectrum of psi_new on the {well.mean():.1%} well-conditioned bins: {rw:.3e}")
+    assert rw <= ONE_STEP_TOL, f"well-conditioned bins: {rw:.3e}"
+    del Fo, Fd
     eg, eo, e32 = g.errors()[0], o.errors()[0], o32.errors()[0]
     assert np.abs(eg[:2] - eo[:2]).max() <= 1e-5            # eps_F, eps_psi: insensitive to those phases
     assert np.abs(eg[2:] - eo[2:]).max() <= max(1e-3, 4 * np.abs(e32[2:] - eo[2:]).max())
@@ -253,6 +308,64 @@ def test_full_size_sampled_views(dm, cfg_i):
     assert rest <= 2e-6 * scale, f"cfg{cfg_i}: zero-data views leave |psi| up to {rest:.3e} (scale {scale:.3e})"
     print(f"cfg{cfg_i} full size, path {g.info()['path']}: sampled-view psi parity ok, zero-data residue {rest / scale:.2e}")
     g.close(); o.close()
+
+
+# (config, raster): FULL-data rasters large enough that the launches take the loop shapes of the full-size runs
+MID = [(1, 20, 20), (2, 30, 30), (3, 20, 20), (4, 10, 10)]
+
+
+def _one_forced_step(dm, pr, what, **params):
+    """One iteration from the oracle's state after its first iteration (cast once to complex64 and loaded on
+    both sides); returns (plan geometry, deviations).  Memory-lean: used up to the full config 2."""
+    g, o = make_pair(dm, pr, **params)
+    o.iterate(1)
+    P32, O32 = o.probe().astype(np.complex64), o.object().astype(np.complex64)
+    psi32 = o.psi().astype(np.complex64)
+    o.set_state(P32, O32, psi32)
+    g.set_state(_t(P32), _t(O32), _t(psi32))
+    del psi32
+    geo = g.geometry()
+    g.iterate(1)
+    o.iterate(1)
+    r = compare_state(g, o, ONE_STEP_TOL, what, lit_pos=pr.positions)
+    eg, eo = g.errors()[-1], o.errors()[-1]
+    assert np.abs(eg - eo).max() <= 1e-5 * max(1.0, np.abs(eo).max()), (eg, eo)
+    g.close(); o.close()
+    return geo, r
+
+
+@pytest.mark.parametrize("cfg_i,ny,nx", MID)
+def test_mid_size_one_step_reaches_full_size_loop_shapes(dm, cfg_i, ny, nx):
+    """S7 / S8 and the persistent psi-update kernels in the loop shapes the full-size runs take, at the 1e-5 bar:
+    (i) every probe-reduction CTA sums >= 5 views (the view-batched loop of probe_partial_kernel AND its tail),
+    (ii) the longest coverage list exceeds one batch of object_gather_kernel (configs 2, 3: second batch runs),
+    (iii) the register-resident kernels give every group of CTAs >= 3 views (prefetch ring, buffer parity flip),
+    (iv) path 4's scratch ring wraps (more views than ring slots).  Geometry read back through dm_plan_geometry."""
+    pr = synth.make_problem(synth.CONFIGS[cfg_i].scaled(ny, nx))
+    geo, r = _one_forced_step(dm, pr, f"cfg{cfg_i} {ny}x{nx}")
+    print(f"cfg{cfg_i} {ny}x{nx}: geometry {geo}; deviations {r}")
+    assert geo["prb_chunk_len"] >= 5, geo
+    if cfg_i in (2, 3):
+        assert geo["obj_max_list"] > geo["obj_batch"], geo
+    if geo["path"] in (3, 5):
+        assert geo["reg_views_per_group"] >= 3, geo
+    if geo["path"] == 4:
+        assert pr.cfg.n_views > geo["wf_slots"], geo
+
+
+@pytest.mark.parametrize("cfg_i", [1, 2])
+def test_full_config_one_step(dm, cfg_i):
+    """The FULL configs 1 (2500 views, K = 2) and 2 (10000 views, K = 4) exactly as bench.py launches them: one
+    iteration from an identical on-trajectory state, psi, P, O and the error row within 1e-5 of the oracle (the
+    oracle holds psi in complex128: 1.2 / 9.8 GiB)."""
+    import psutil
+    need = {1: 8, 2: 48}[cfg_i] * 2 ** 30
+    if psutil.virtual_memory().available < need:
+        pytest.skip(f"full config {cfg_i} needs ~{need >> 30} GiB of host memory for the FP64 oracle state")
+    pr = synth.make_problem(cfg_i)
+    geo, r = _one_forced_step(dm, pr, f"full cfg{cfg_i}")
+    print(f"full cfg{cfg_i}: geometry {geo}; deviations {r}")
+    assert geo["prb_chunk_len"] >= 5 and geo["reg_views_per_group"] >= 3, geo
 
 
 @pytest.mark.parametrize("N,K,L,ny,nx", [(128, 4, 2, 3, 3), (128, 3, 1, 4, 3), (128, 1, 1, 5, 4), (128, 1, 5, 2, 3),
