@@ -60,7 +60,10 @@ typedef enum {
                                  dm_set_data if N > 128), 3 = force the register-resident
                                  path (DM_ERR_UNSUPPORTED at dm_set_data unless N = 128),
                                  4 = force the view-pipelined warp-FFT path (any N; the
-                                 default for N >= 256)                                       */
+                                 default for N >= 256), 5 = force the register-resident
+                                 path on clusters of two 256-thread CTAs, two CTAs per SM
+                                 (N = 128 only; measured slower than path 3, kept as the
+                                 record of that experiment)                   */
     DM_PARAM_LAG = 5,         /* path 4: views between the row, column and inverse-row phases
                                  of one view (integer >= 1; 0 = derive from the task counts,
                                  default).  Sizes the scratch ring: set before
@@ -155,8 +158,9 @@ dm_status dm_solve_host(dm_plan *plan, const float *intensities_host, const floa
                         const float *object0_host, int n_iter, float *out_probe_host,
                         float *out_object_host, void *stream);
 
-/* Which path dm_iterate runs for this plan: 1 staged, 2 fused, 3 register-resident (valid
- * after dm_set_data);
+/* Which path dm_iterate runs for this plan: 1 staged, 2 fused, 3 register-resident,
+ * 4 view-pipelined warp-FFT, 5 register-resident on CTA pairs, 64 FP64 validation mode
+ * (valid after dm_set_data);
  * and how many kernels one iteration launches (the bench's gpu_launches claim).           */
 dm_status dm_plan_info(const dm_plan *plan, int *path, int *launches_per_iter);
 

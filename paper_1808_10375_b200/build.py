@@ -43,7 +43,8 @@ def build(force: bool = False, verbose: bool = False) -> str:
     if not force and up_to_date():
         return LIB
     nvcc = os.environ.get("NVCC", "nvcc")
-    cmd = [nvcc] + NVCC_FLAGS + sources() + ["-o", LIB + ".tmp"]
+    # DM_NVCC_EXTRA: extra nvcc flags (e.g. -DDM_PAIR_PROF, the clock64 phase profile of dm_pairfft.cuh)
+    cmd = [nvcc] + NVCC_FLAGS + os.environ.get("DM_NVCC_EXTRA", "").split() + sources() + ["-o", LIB + ".tmp"]
     res = subprocess.run(cmd, stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True)
     log = os.path.join(HERE, "build.log")
     with open(log, "w") as f:
