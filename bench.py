@@ -59,6 +59,9 @@ def measured_traffic(workload: str, path: int, lag: int):
                                          "csrc_digest": e.get("csrc_digest"), "kind": "committed ncu capture, not measured in this run"}
 
 
+# FP32 lane-operations (FADD / FMUL / FFMA lanes, packed counted twice) per pixel and mode of the psi update:
+# 2 N-point FFT pairs (forward + inverse, ~5.5 log2(N^2) each after FMA fusion) + ~30 elementwise
+LANE_OPS_PER_PIXEL = {64: 98, 128: 109, 256: 120, 512: 132}
 NOMINAL_HBM_GBS = 8000.0      # north_star / SURVEY.md 8(d): "~8 TB/s"
 
 
@@ -288,6 +291,8 @@ def run_ours(args, cfg):
             torch.cuda.empty_cache()
             per_config.append(r2)
     clocks = sampler.stop()
+    # FP32 / HBM / L2 / shared-memory rates of this device, measured by the library's own streaming kernels
+    device_peaks = dm.measure_peaks() if world == 1 else None
 
     if rank != 0:
         grp.close()
@@ -301,6 +306,18 @@ def run_ours(args, cfg):
                    "ms_per_step": ms_e2e / e2e_steps, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                    "call": "dm_solve_host(n_iter=1): H2D intensities+P0+O0 (pinned), set_data, 1 iteration, D2H P+O"}
     head["clocks"] = clocks
+    if device_peaks:
+        head["device_peaks"] = device_peaks
+        for r in [head] + per_config:
+            # the second roof of north_star: FFT + elementwise lane-operations over the measured FP32 issue rate
+            # (an FMA = one lane-operation; LANE_OPS_PER_PIXEL from ncu's FMA-pipe cycles)
+            c = r["config"]
+            ops = LANE_OPS_PER_PIXEL[c["N"]] * c["mode_views"] * c["N"] ** 2
+            t = r["roofline"]["ms_per_launch"] * 1e-3
+            r["roofline_fp32"] = {"bound": "alu", "kernel": "psi update (S1-S6)", "achieved": ops / t / 1e12,
+                                  "peak": device_peaks["fp32_lane_ops_per_s_ffma2"] / 1e12, "unit": "T lane-op/s",
+                                  "frac": ops / t / device_peaks["fp32_lane_ops_per_s_ffma2"],
+                                  "lane_ops_per_pixel_mode": LANE_OPS_PER_PIXEL[c["N"]]}
     if per_config:
         head["per_config"] = per_config
     line = head
@@ -337,9 +354,19 @@ def main():
     ap.add_argument("--ref-mode-views", type=int, default=4096,
                     help="size of the bounded oracle sample (mode-views per iteration)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--peaks", action="store_true", help="only measure and print the device rates of dm_measure_peaks")
     args = ap.parse_args()
     if args.print_csrc_digest:
         print(csrc_digest())
+        return
+    if args.peaks:
+        import torch
+        from paper_1808_10375_b200 import dm
+        assert torch.cuda.is_available(), "bench.py --peaks needs a CUDA device"
+        sampler = ClockSampler(0)
+        sampler.start()
+        pk = dm.measure_peaks()
+        print(json.dumps({"device_peaks": pk, "clocks": sampler.stop(), "gpu": torch.cuda.get_device_name(0)}), flush=True)
         return
     from paper_1808_10375_b200 import synth
     cfg = synth.CONFIGS[args.config]

@@ -185,6 +185,18 @@ dm_status dm_plan_geometry(const dm_plan *plan, int32_t *out_host, int n_out);
 dm_status dm_plan_set_profiling(dm_plan *plan, int on);
 dm_status dm_get_phase_ms(dm_plan *plan, float *out_ms4, int *iters);
 
+/* Measurement aid (no plan needed): the roofline denominators of DESIGN.md measured on the current
+ * device with plain streaming kernels ("FP32 peak").  scratch_dev = DEV buffer of
+ * scratch_bytes >= 512 MiB (>> L2; contents destroyed), 16-byte aligned.  Writes min(n_out,
+ * DM_PEAK_FIELDS) f64 to out_host (HOST) and SYNCS:
+ *   [0] FP32 lane-operations/s with scalar FFMA     [1] the same with packed FFMA2 (fma.rn.f32x2)
+ *   [2] HBM read-only GB/s   [3] HBM copy GB/s (read + write bytes)   [4] L2-resident read GB/s (32 MiB)
+ *   [5] shared-memory read GB/s (conflict-free 128-bit)   [6] SM count
+ * One FMA counts as ONE lane-operation: an FFT butterfly is mostly adds, so the FP32 bound of the psi
+ * update is lane-operations / [0], not flops / (2 x [0]).  Errors: INVALID_ARG, WORKSPACE, CUDA.        */
+#define DM_PEAK_FIELDS 7
+dm_status dm_measure_peaks(void *scratch_dev, size_t scratch_bytes, double *out_host, int n_out, void *stream);
+
 /* Test hook, HOST only, no CUDA call: runs the kernels' own FFT pass code (the same
  * __host__ __device__ functions the kernels inline: radix butterflies, twiddle table,
  * swizzled tile addressing, digit-reversal map) single-threaded on the host for one

@@ -24,7 +24,7 @@ SYMBOLS = (
     "dm_plan_create", "dm_plan_set_param", "dm_plan_workspace_bytes", "dm_plan_set_workspace",
     "dm_set_data", "dm_iterate", "dm_get_probe", "dm_get_object", "dm_get_psi", "dm_get_errors",
     "dm_set_state", "dm_get_window_table", "dm_get_coverage", "dm_get_alphas", "dm_get_mode_power", "dm_solve_host",
-    "dm_plan_info", "dm_plan_geometry", "dm_plan_set_profiling", "dm_get_phase_ms", "dm_host_fft2", "dm_host_fft2_path", "dm_status_string", "dm_last_error", "dm_plan_destroy",
+    "dm_plan_info", "dm_plan_geometry", "dm_plan_set_profiling", "dm_get_phase_ms", "dm_measure_peaks", "dm_host_fft2", "dm_host_fft2_path", "dm_status_string", "dm_last_error", "dm_plan_destroy",
 )
 
 _vp, _int, _dbl = C.c_void_p, C.c_int, C.c_double
@@ -65,6 +65,7 @@ def lib() -> C.CDLL:
         L.dm_plan_geometry.argtypes = [_vp, _vp, _int]
         L.dm_plan_set_profiling.argtypes = [_vp, _int]
         L.dm_get_phase_ms.argtypes = [_vp, _vp, C.POINTER(_int)]
+        L.dm_measure_peaks.argtypes = [_vp, C.c_size_t, _vp, _int, _vp]
         L.dm_host_fft2.argtypes = [_int, _vp, _vp, _int]
         L.dm_host_fft2_path.argtypes = [_int, _int, _vp, _vp, _int]
         L.dm_status_string.argtypes = [_int]
@@ -82,6 +83,21 @@ def lib() -> C.CDLL:
 
 def _np_ptr(a: np.ndarray):
     return a.ctypes.data_as(_vp)
+
+
+PEAK_FIELDS = ("fp32_lane_ops_per_s_ffma", "fp32_lane_ops_per_s_ffma2", "hbm_read_gbs", "hbm_copy_gbs", "l2_read_gbs",
+               "smem_read_gbs", "sms")
+
+
+def measure_peaks(scratch_bytes: int = 2 << 30) -> dict:
+    """dm_measure_peaks: FP32 / HBM / L2 / shared-memory rates of the current CUDA device (syncs)."""
+    import torch
+    buf = torch.empty(scratch_bytes, dtype=torch.uint8, device="cuda")
+    out = np.zeros(len(PEAK_FIELDS), dtype=np.float64)
+    st = lib().dm_measure_peaks(_vp(buf.data_ptr()), scratch_bytes, _np_ptr(out), len(out), _vp(torch.cuda.current_stream().cuda_stream))
+    if st != 0:
+        raise DMError(st, "dm_measure_peaks")
+    return dict(zip(PEAK_FIELDS, (float(v) for v in out)))
 
 
 def host_fft2(x: np.ndarray, inverse: bool = False, path: int = 0) -> np.ndarray:
