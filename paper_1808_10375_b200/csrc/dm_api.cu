@@ -12,7 +12,6 @@
 #include "../../include/dm.h"
 #include "dm_kernels.cuh"
 #include "dm_pairfft.cuh"
-#include "dm_vtfft.cuh"
 #include "dm_fp64.cuh"
 
 namespace {
@@ -454,59 +453,6 @@ dm_status launch_pairfft(dm_plan *plan, cudaStream_t st, bool query_only)
     }
 }
 
-// path 6: two whole frames per SM, each on a 256-thread CTA that plays 512 virtual threads (dm_vtfft.cuh)
-template <int MT> dm_status launch_vtfft_t(dm_plan *plan, cudaStream_t st, bool query_only)
-{
-    auto kern = dmvt::vtfft128_kernel<MT>;
-    if (query_only) {
-        CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, dmvt::VT_SMEM));
-        CU(cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
-        // residency from the device limits (the occupancy API reports one block per SM for kernels that allocate
-        // tensor memory, see launch_pairfft_t); the frames of a view wait on one another, so all CTAs must be resident
-        int dev = 0, sms = 0, smem_sm = 0, regs_sm = 0;
-        cudaFuncAttributes fa;
-        CU(cudaGetDevice(&dev));
-        CU(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
-        CU(cudaDeviceGetAttribute(&smem_sm, cudaDevAttrMaxSharedMemoryPerMultiprocessor, dev));
-        CU(cudaDeviceGetAttribute(&regs_sm, cudaDevAttrMaxRegistersPerMultiprocessor, dev));
-        CU(cudaFuncGetAttributes(&fa, kern));
-        const size_t smem_cta = (size_t)dmvt::VT_SMEM + fa.sharedSizeBytes + 1024;
-        int per = 2;                                                // 2 x 256 tensor-memory columns
-        if ((size_t)per * smem_cta > (size_t)smem_sm) per = (int)((size_t)smem_sm / smem_cta);
-        if (per * fa.numRegs * dmvt::VNT > regs_sm) per = regs_sm / (fa.numRegs * dmvt::VNT);
-        int slots = sms * per;
-        if (slots > plan->reg_cap) slots = plan->reg_cap;
-        int groups = slots / plan->M;
-        if (groups < 1) return fail(plan, DM_ERR_UNSUPPORTED, "virtual-thread kernel: %d CTAs fit the device, a view needs %d", slots, plan->M);
-        if (groups > plan->n_views) groups = plan->n_views;
-        plan->reg_grid = groups * plan->M;
-        plan->reg_sw = plan->M > 1;
-        return DM_OK;
-    }
-    dmvt::VtArgs a;
-    memset(&a, 0, sizeof a);
-    a.n_views = plan->n_views; a.K = plan->K; a.L = plan->L; a.H = plan->H; a.W = plan->W;
-    a.pos = plan->pos_d; a.P = plan->Pbuf[plan->curP]; a.O = plan->Obuf[plan->curO];
-    a.psi = plan->psi; a.amp = plan->amp; a.wy = plan->wy_d; a.wx = plan->wx_d;
-    a.sbuf = plan->sbuf; a.part = plan->partA; a.gbar = plan->reg_gbar;
-    a.beta = (float)plan->beta; a.eps = (float)plan->eps_f;
-    if (plan->M > 1) CU(cudaMemsetAsync(plan->reg_gbar, 0, (size_t)plan->reg_cap * sizeof(int), st));
-    kern<<<plan->reg_grid, dmvt::VNT, dmvt::VT_SMEM, st>>>(a);
-    CU(cudaGetLastError());
-    return DM_OK;
-}
-
-dm_status launch_vtfft(dm_plan *plan, cudaStream_t st, bool query_only)
-{
-    switch (plan->M) {
-    case 1: return launch_vtfft_t<1>(plan, st, query_only);
-    case 2: return launch_vtfft_t<2>(plan, st, query_only);
-    case 3: return launch_vtfft_t<3>(plan, st, query_only);
-    case 4: return launch_vtfft_t<4>(plan, st, query_only);
-    default: return launch_vtfft_t<0>(plan, st, query_only);
-    }
-}
-
 // path 4: persistent task-queue kernel (rows -> columns + modulus -> rows through an L2-resident ring)
 template <int N> dm_status launch_wf_t(dm_plan *plan, cudaStream_t st, bool query_only)
 {
@@ -557,7 +503,6 @@ dm_status launch_psi_update(dm_plan *plan, cudaStream_t st, bool prepare = false
     if (plan->path == 4) return launch_wf(plan, st, prepare);
     if (plan->path == 3) return launch_regfft(plan, st, prepare);
     if (plan->path == 5) return launch_pairfft(plan, st, prepare);
-    if (plan->path == 6) return launch_vtfft(plan, st, prepare);
     if (plan->path == 2) {
         if (plan->N == 64) return launch_fused<64, 256>(plan, st, prepare);
         return launch_fused<128, 512>(plan, st, prepare);
@@ -701,7 +646,7 @@ dm_status dm_plan_set_param(dm_plan *plan, dm_param which, double v)
     case DM_PARAM_ALPHA_OBJ: if (v < 0) break; plan->a_obj = v; return DM_OK;
     case DM_PARAM_ALPHA_PROBE: if (v < 0) break; plan->a_probe = v; return DM_OK;
     case DM_PARAM_EPS_F: if (v < 0) break; plan->eps_f = v; return DM_OK;
-    case DM_PARAM_PATH: if (v != 0 && v != 1 && v != 2 && v != 3 && v != 4 && v != 5 && v != 6) break; plan->path_req = (int)v; return DM_OK;
+    case DM_PARAM_PATH: if (v != 0 && v != 1 && v != 2 && v != 3 && v != 4 && v != 5) break; plan->path_req = (int)v; return DM_OK;
     case DM_PARAM_PRECISION:
         if (v != 0 && v != 1) break;
         if (plan->ws) return fail(plan, DM_ERR_INVALID_ARG, "the precision sizes the workspace: set it before dm_plan_set_workspace");
@@ -860,7 +805,7 @@ dm_status set_data_impl(dm_plan *plan, const float *intensities, const float *pr
     if (plan->precision == 1) path = 64;         // FP64 validation mode: its own plain kernels
     if (path == 2 && plan->N > 128)
         return fail(plan, DM_ERR_UNSUPPORTED, "fused per-frame path needs N <= 128 (N = %d)", plan->N);
-    if ((path == 3 || path == 5 || path == 6) && plan->N != 128)
+    if ((path == 3 || path == 5) && plan->N != 128)
         return fail(plan, DM_ERR_UNSUPPORTED, "register-resident paths need N = 128 (N = %d)", plan->N);
     plan->path = path;
     cudaStream_t st = (cudaStream_t)stream;
@@ -870,7 +815,7 @@ dm_status set_data_impl(dm_plan *plan, const float *intensities, const float *pr
     // intensities of dm_solve_host on the copy engine)
     if (plan->tables_path != path) {
     plan->spec.assign(NN, 0);
-    if (path == 3 || path == 5 || path == 6) {
+    if (path == 3 || path == 5) {
         for (int tid = 0; tid < dmreg::RNT; ++tid)
             for (int e = 0; e < dmreg::REPT; ++e) plan->spec[dmreg::spec_pos(tid, e)] = dmreg::spec_freq(tid, e);
         std::vector<float> wy(256), wx(256);
@@ -1015,7 +960,7 @@ dm_status dm_iterate(dm_plan *plan, int n_iter, void *stream)
         if (plan->path == 4) {
             e.pF = plan->partA; e.nF = plan->n_views * plan->wf_nB; e.sF = 2;
             e.pS = plan->partB; e.nS = plan->n_views * plan->wf_nC; e.sS = 2;
-        } else if (plan->path == 3 || plan->path == 5 || plan->path == 6) {
+        } else if (plan->path == 3 || plan->path == 5) {
             e.pF = plan->partA;     e.nF = plan->reg_grid; e.sF = 4;
             e.pS = plan->partA + 2; e.nS = plan->reg_grid; e.sS = 4;
         } else if (plan->path == 2) {
@@ -1271,7 +1216,7 @@ dm_status dm_plan_geometry(const dm_plan *plan, int32_t *out_host, int n_out)
     if (!plan || !out_host || n_out < 0) return DM_ERR_INVALID_ARG;
     int path = 0;
     dm_plan_info(plan, &path, nullptr);
-    const bool reg = path == 3 || path == 5 || path == 6;
+    const bool reg = path == 3 || path == 5;
     const int per_view = path == 5 ? 2 * plan->M : plan->M;
     const int clusters = reg && plan->reg_grid > 0 ? plan->reg_grid / per_view : 0;
     const int32_t g[DM_GEOMETRY_FIELDS] = {
