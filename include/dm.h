@@ -103,8 +103,11 @@ dm_status dm_plan_set_workspace(dm_plan *plan, void *dev, size_t bytes);
  * copies P0 and O0, sets psi_jkl = P0_k * O0_l|window, freezes the absolute regularisers
  * from P0/O0 (reading A8), uploads the tables and clears the error table.
  * intensities DEV f32 [n_views][N][N] (>= 0, not validated on the device),
- * probe0 DEV c64 [K][N][N], object0 DEV c64 [L][obj_h][obj_w].  Async on `stream`; the
- * caller's buffers may be released once that stream work has completed.                */
+ * probe0 DEV c64 [K][N][N], object0 DEV c64 [L][obj_h][obj_w].  Work is enqueued on `stream`;
+ * the caller's buffers may be released once that stream work has completed.  The FIRST call
+ * on a workspace (and the first after a change of path or precision) also uploads the integer
+ * tables and twiddles from pageable host memory and SYNCS `stream` (up to three times) while
+ * doing so; later calls on the same workspace are fully asynchronous.                    */
 dm_status dm_set_data(dm_plan *plan, const float *intensities, const float *probe0,
                       const float *object0, void *stream);
 
@@ -143,7 +146,9 @@ dm_status dm_get_alphas(const dm_plan *plan, double *out_host2);
 /* Mode diagnostics (a probe mode is kept while its "contribution ... to the total
  * intensity is larger than at least 1%"): the power fraction of every mode of the current
  * state, out_host[k] = sum_r |P_k|^2 / sum_k sum_r |P_k|^2 (k < K) followed by the same for the
- * object modes, out_host[K + l]; f64[K + L] to HOST; 0/0 := 0.  Fixed-order FP64 sums.  SYNCS.  */
+ * object modes, out_host[K + l]; f64[K + L] to HOST; 0/0 := 0.  Fixed-order FP64 sums.  SYNCS THE
+ * DEVICE (cudaDeviceSynchronize) first, so it sees the state of whatever stream dm_iterate ran on, then
+ * runs its two small kernels on the default stream and syncs again: a diagnostic, not a hot-path call.  */
 dm_status dm_get_mode_power(const dm_plan *plan, double *out_host);
 
 /* End-to-end entry with HOST buffers (what a beamline caller with data in host memory

@@ -313,6 +313,14 @@ __device__ __forceinline__ void bulk_load(void *dst_smem, const void *src_gmem, 
 __device__ __forceinline__ void cluster_arrive() { asm volatile("barrier.cluster.arrive.release.aligned;\n" ::: "memory"); }
 __device__ __forceinline__ void cluster_wait() { asm volatile("barrier.cluster.wait.acquire.aligned;\n" ::: "memory"); }
 
+// -DDM_REG_PROF (DM_NVCC_EXTRA of build.py): thread 0 of CTAs 0, 1 and 100 accumulates clock64 per phase and prints the
+// mean cycles per frame at the end of the launch (the table of DESIGN.md 6.1; measurement builds only)
+#ifdef DM_REG_PROF
+#define RPROF(i) { const long long now_ = clock64(); prof[i] += now_ - tprev; tprev = now_; }
+#else
+#define RPROF(i)
+#endif
+
 // Persistent CTAs; cluster = the M = K*L mode frames of one view (cluster rank m = mode index),
 // cluster c processes views c, c + n_clusters, ...  MT = compile-time M (0: run-time M).
 template <int MT>
@@ -364,6 +372,9 @@ __global__ void __launch_bounds__(RNT, 1) regfft128_kernel(const RegArgs a)
         bulk_load(pbuf + 65536, src + 65536, 65536, &mb_hi);
     }
 
+#ifdef DM_REG_PROF
+    long long prof[8] = {0, 0, 0, 0, 0, 0, 0, 0}, tprev = clock64();
+#endif
     int it = 0;
     for (int view = cl; view < a.n_views; view += ncl, par ^= 1, ++it) {
         const int2 p0 = a.pos[view];
@@ -407,6 +418,7 @@ __global__ void __launch_bounds__(RNT, 1) regfft128_kernel(const RegArgs a)
             }
         }
         __syncthreads();                    // the whole prefetch buffer has been read
+        RPROF(0)
         if (tid == 0) {
             bulk_load(pbuf, a.amp + (size_t)view * RNN, 65536, &mb_amp);
             if (nview < a.n_views) bulk_load(pbuf + 65536, nsrc + 65536, 65536, &mb_hi);
@@ -437,6 +449,7 @@ __global__ void __launch_bounds__(RNT, 1) regfft128_kernel(const RegArgs a)
             x2_read(u, z, w, t, xb2);
         }
         pass3<false>(u);
+        RPROF(1)
         // ---- S4: mode-summed modulus constraint (|F|^2 exchanged through L2) ----
         {
             float4 *mine = a.sbuf + (((size_t)par * gridDim.x + blockIdx.x) * 8) * RNT + tid;
@@ -465,6 +478,7 @@ __global__ void __launch_bounds__(RNT, 1) regfft128_kernel(const RegArgs a)
             } else {
                 __syncthreads();
             }
+            RPROF(2)
             mbar_wait(&mb_amp, par);
             const float4 *ampv = reinterpret_cast<const float4 *>(pbuf) + tid;
             const float4 *peers = a.sbuf + (((size_t)par * gridDim.x + (size_t)cl * M) * 8) * RNT + tid;
@@ -508,6 +522,7 @@ __global__ void __launch_bounds__(RNT, 1) regfft128_kernel(const RegArgs a)
                 }
             }
         }
+        RPROF(3)
         // ---- S5: inverse 2-D FFT (mirror) ----
         pass3<true>(u);
 #pragma unroll
@@ -536,6 +551,7 @@ __global__ void __launch_bounds__(RNT, 1) regfft128_kernel(const RegArgs a)
             for (int r = 0; r < 4; ++r) wx[r] = s_wx[t * 4 + r];
             pass1_inv(u, wy, wx);
         }
+        RPROF(4)
         // ---- S6: psi_new = psi_old + beta (G - P O) ----
 #pragma unroll
         for (int i = 0; i < 8; i += 2) {
@@ -555,7 +571,13 @@ __global__ void __launch_bounds__(RNT, 1) regfft128_kernel(const RegArgs a)
                 psi_f[(e >> 2) * 16 * RN + (e & 3) * 32] = nw;
             }
         }
+        RPROF(5)
     }
+#ifdef DM_REG_PROF
+    if (tid == 0 && it > 0 && (blockIdx.x == 0 || blockIdx.x == 1 || blockIdx.x == 100))
+        printf("regfft128 blk %d, %d frames: S1+S2 %lld | forward FFT %lld | S4 store + group barrier %lld | S4 peers + scaling %lld | inverse FFT %lld | S6 %lld cycles per frame\n",
+               blockIdx.x, it, prof[0] / it, prof[1] / it, prof[2] / it, prof[3] / it, prof[4] / it, prof[5] / it);
+#endif
     asm volatile("tcgen05.fence::before_thread_sync;\n" ::: "memory");
     __syncthreads();
     if (w == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;\n" :: "r"(s_tmem), "r"(512) : "memory");
