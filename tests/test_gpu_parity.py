@@ -112,11 +112,14 @@ def test_one_iteration_parity(dm, cfg_i, ny, nx, path):
     """P2: set_data state (psi = P0*O0, frozen alphas) is exact; then one full iteration from an
     identical on-trajectory state (oracle state after 1 iteration) within 1e-5 on psi, P, O.
     path 0 = what dm_iterate picks (register-resident kernel for N = 128, fused shared-memory
-    kernel for N = 64, view-pipelined warp-FFT kernel above); 1, 2, 3, 4 force the staged /
-    fused / register-resident / warp-FFT path."""
+    kernel for N = 64, view-pipelined warp-FFT kernel above); 1, 2, 3, 4, 5 force the staged /
+    fused / register-resident / warp-FFT / CTA-pair register-resident path."""
     N = synth.CONFIGS[cfg_i].N
     if (path == 2 and N > 128) or (path in (3, 5) and N != 128):
         pytest.skip("path not defined for this frame size")
+    if path == 1 and cfg_i not in (0, 3):
+        pytest.skip("path 1 (the first, staged kernels; no configuration defaults to it) is kept as a cross-check on one "
+                    "small and one large frame size only")
     pr = synth.make_problem(synth.CONFIGS[cfg_i].scaled(ny, nx))
     g, o = make_pair(dm, pr, path=path)
     compare_state(g, o, 1e-6, "t=0")                         # psi init is one complex multiply
@@ -353,6 +356,16 @@ def test_mid_size_one_step_reaches_full_size_loop_shapes(dm, cfg_i, ny, nx):
         assert pr.cfg.n_views > geo["wf_slots"], geo
 
 
+@pytest.mark.parametrize("cfg_i,ny,nx", [(1, 20, 20), (2, 30, 30)])
+def test_mid_size_one_step_path5(dm, cfg_i, ny, nx):
+    """The same mid-size one-step comparison for the CTA-pair kernel (path 5): every cluster takes >= 3 views, so
+    its prefetch ring, the exchange-2 barrier parity and the group barrier counters all wrap."""
+    pr = synth.make_problem(synth.CONFIGS[cfg_i].scaled(ny, nx))
+    geo, r = _one_forced_step(dm, pr, f"cfg{cfg_i} {ny}x{nx} path 5", path=5)
+    print(f"cfg{cfg_i} {ny}x{nx} path 5: geometry {geo}; deviations {r}")
+    assert geo["path"] == 5 and geo["reg_views_per_group"] >= 3, geo
+
+
 @pytest.mark.parametrize("cfg_i", [1, 2])
 def test_full_config_one_step(dm, cfg_i):
     """The FULL configs 1 (2500 views, K = 2) and 2 (10000 views, K = 4) exactly as bench.py launches them: one
@@ -482,3 +495,19 @@ def test_full_config1_50_iterations(dm):
         if kw:
             assert rP <= 1e-3 and rO <= 1e-3 and curve_psi <= 1e-3
         g.close()
+
+
+def test_measure_peaks_is_sane(dm):
+    """dm_measure_peaks (the roofline denominators): every rate is positive and ordered the way the memory hierarchy
+    is (shared memory and L2-resident reads above HBM reads, HBM copy within 2x of HBM read), the two FP32 figures
+    agree within 20 %, and the argument checks fire."""
+    import ctypes as C
+    pk = dm.measure_peaks(1 << 30)
+    print("device peaks", pk)
+    assert all(v > 0 for v in pk.values()), pk
+    assert pk["l2_read_gbs"] > pk["hbm_read_gbs"] > 0.5 * pk["hbm_copy_gbs"], pk
+    assert pk["hbm_copy_gbs"] > 0.5 * pk["hbm_read_gbs"], pk
+    assert pk["smem_read_gbs"] > pk["hbm_read_gbs"], pk
+    assert abs(pk["fp32_lane_ops_per_s_ffma2"] / pk["fp32_lane_ops_per_s_ffma"] - 1.0) < 0.2, pk
+    out = np.zeros(7)
+    assert dm.lib().dm_measure_peaks(None, 1 << 30, out.ctypes.data_as(C.c_void_p), 7, None) == 1      # INVALID_ARG
