@@ -40,7 +40,7 @@ struct dm_plan {
     int path_req, path;                  // requested / chosen (1 staged, 2 fused, 3 register-resident)
     int reg_grid;                        // path 3: number of persistent CTAs (multiple of M)
     bool reg_sw;                         // path 3: software group barrier instead of a hardware cluster
-    int *reg_gbar;                       // path 3: [reg_cap] group barrier counters
+    int *reg_gbar;                       // paths 3, 5: [reg_cap] group barrier counters + 1 sticky "a CTA gave up waiting" flag (path 5)
     int reg_cap;                         // paths 3, 5: upper bound on resident CTAs (2 per SM)
     // path 4 (dm_warpfft.cuh): ring slots, phase lag (views), tasks per view and phase, persistent CTAs
     int wf_S, wf_D, wf_nA, wf_nB, wf_nC, wf_grid, wf_nw;
@@ -222,7 +222,7 @@ size_t carve(dm_plan *p, unsigned char *base)
     p->wy_d = (float2 *)take(128 * sizeof(float2));
     p->wx_d = (float2 *)take(128 * sizeof(float2));
     p->sbuf = (float4 *)take(p->N == 128 ? (size_t)2 * p->reg_cap * 8 * dmreg::RNT * sizeof(float4) : 0);
-    p->reg_gbar = (int *)take((size_t)p->reg_cap * sizeof(int));
+    p->reg_gbar = (int *)take(((size_t)p->reg_cap + 1) * sizeof(int));
     p->tw_d = (float2 *)take(p->N * sizeof(float2));
     p->mode_pow = (double *)take((size_t)(p->K + p->L) * sizeof(double));
     p->errors = (double *)take((size_t)ERR_ROWS_CAP * (2 + p->K + p->L) * sizeof(double));
@@ -434,7 +434,7 @@ template <int MT> dm_status launch_pairfft_t(dm_plan *plan, cudaStream_t st, boo
     a.n_views = plan->n_views; a.K = plan->K; a.L = plan->L; a.H = plan->H; a.W = plan->W;
     a.pos = plan->pos_d; a.P = plan->Pbuf[plan->curP]; a.O = plan->Obuf[plan->curO];
     a.psi = plan->psi; a.amp = plan->amp; a.wy = plan->wy_d; a.wx = plan->wx_d;
-    a.sbuf = plan->sbuf; a.part = plan->partA; a.gbar = plan->reg_gbar;
+    a.sbuf = plan->sbuf; a.part = plan->partA; a.gbar = plan->reg_gbar; a.gave_up = plan->reg_gbar + plan->reg_cap;
     a.beta = (float)plan->beta; a.eps = (float)plan->eps_f;
     cfg.gridDim = dim3((unsigned)plan->reg_grid);
     if (plan->M > 1) CU(cudaMemsetAsync(plan->reg_gbar, 0, (size_t)plan->reg_cap * sizeof(int), st));
@@ -886,6 +886,7 @@ dm_status set_data_impl(dm_plan *plan, const float *intensities, const float *pr
     CU(cudaMemcpyAsync(plan->Pbuf[0], probe0, plan->K * NN * sizeof(float2), cudaMemcpyDeviceToDevice, st));
     CU(cudaMemcpyAsync(plan->Obuf[0], object0, plan->L * HW * sizeof(float2), cudaMemcpyDeviceToDevice, st));
     CU(cudaMemsetAsync(plan->alphas, 0, 2 * sizeof(float), st));
+    CU(cudaMemsetAsync(plan->reg_gbar + plan->reg_cap, 0, sizeof(int), st));
     const size_t total = (size_t)plan->n_views * NN;
     if (n_chunks <= 0) amp_permute_kernel<<<plan->sms * 8, 256, 0, st>>>(plan->N, intensities, plan->spec_d, plan->amp, total);
     psi_init_kernel<<<dim3((unsigned)((NN + 1023) / 1024), (unsigned)(plan->n_views * plan->M)), 256, 0, st>>>(
@@ -1038,6 +1039,11 @@ dm_status dm_get_errors(const dm_plan *plan, double *out_host, int max_rows, int
     if (s != DM_OK) return s;
     if (!out_host || !rows_written || max_rows < 0) return fail(plan, DM_ERR_INVALID_ARG, "bad output arguments");
     CU(cudaDeviceSynchronize());
+    if (plan->path == 5) {      // the pair kernel's CTAs wait on one another; one that gave up (grid not resident) leaves garbage
+        int gave_up = 0;
+        CU(cudaMemcpy(&gave_up, plan->reg_gbar + plan->reg_cap, sizeof(int), cudaMemcpyDeviceToHost));
+        if (gave_up) return fail(plan, DM_ERR_CUDA, "path 5: a CTA timed out at the group barrier (its grid was not resident); results are invalid");
+    }
     const int n = plan->rows < max_rows ? plan->rows : max_rows;
     if (n > 0) CU(cudaMemcpy(out_host, plan->errors, (size_t)n * (2 + plan->K + plan->L) * sizeof(double), cudaMemcpyDeviceToHost));
     *rows_written = n;

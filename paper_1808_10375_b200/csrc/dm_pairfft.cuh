@@ -144,6 +144,7 @@ struct PairArgs {
     float *part;                // [grid][4]
     float beta, eps;
     int *gbar;                  // [groups] arrival counters of the 2 M CTAs of a view
+    int *gave_up;               // sticky flag: set when a CTA stops waiting at the group barrier (dm_get_errors reports it)
 };
 
 // grid = 2 * (frames in flight); cluster (2,1,1); frame slot f = blockIdx.x / 2 holds mode f % M of the
@@ -304,7 +305,7 @@ __global__ void __launch_bounds__(PNT, 2) pairfft128_kernel(const PairArgs a)
                     do {
                         asm volatile("ld.acquire.gpu.global.s32 %0, [%1];\n" : "=r"(v) : "l"(a.gbar + cl) : "memory");
                     } while (v < want && ++spins < SPIN_LIMIT);
-                    if (v < want) alive = false;
+                    if (v < want) { alive = false; atomicExch(a.gave_up, 1); }
                 }
                 __syncthreads();
             }

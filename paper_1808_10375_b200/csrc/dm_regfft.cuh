@@ -35,7 +35,13 @@ using namespace dmfft;
 constexpr int RN = 128, RNN = RN * RN, RNT = 512, REPT = 32;
 // exchange buffer: 16 warps x (2 blocks of 16 rows x 144 B) for exchange 1, 64 KiB for exchange 2
 constexpr int X1_ROW = 144, X1_BLK = 16 * X1_ROW, X1_WARP = 2 * X1_BLK;       // bytes
-constexpr int XBUF_BYTES = 16 * X1_WARP;                                       // 73728 >= 65536
+constexpr int XBUF_BYTES = 16 * X1_WARP;                                       // 73728 >= 65536 (contiguous exchange-1 regions: path 5, host emulation)
+// path 3 keeps a warp's exchange-1 rows inside the 4 KiB that the same warp reads in exchange 2 (rows 0..27) plus a
+// private spare strip behind the 64 KiB (rows 28..31), so exchange 1 never touches what another warp still has to
+// read: no block barrier between exchange 2 and exchange 1.  Spare strips start at 64 (mod 128) bytes: the 128-bit
+// loads of rows 24..27 (main) and 28..31 (spare) then fall on disjoint banks.
+constexpr int X1S_MAIN_ROWS = 28, X1S_SPARE = 640, X1S_SPARE_OFF = 65536 + 64;
+constexpr int XBUF3_BYTES = X1S_SPARE_OFF + 16 * X1S_SPARE;                       // 75840
 
 // cos / sin of 2 pi m / 32
 __device__ __host__ constexpr float c32(int m)
@@ -131,6 +137,16 @@ DM_HD void pass1_inv(float2 (&u)[32], const float2 *wy, const float2 *wx)
 
 template <bool INV> DM_HD void pass2(float2 (&u)[32]) { dft32<INV>(u); }
 
+// pass 3 works on the two register halves z = 0, 1 independently (they are also the two rounds of exchange 2)
+template <bool INV> DM_HD void pass3_half(float2 (&u)[32], int z)
+{
+    float2 v[16];
+#pragma unroll
+    for (int i = 0; i < 16; ++i) v[i] = u[16 * z + i];
+    dft16<INV>(v);
+#pragma unroll
+    for (int i = 0; i < 16; ++i) u[16 * z + i] = v[i];
+}
 template <bool INV> DM_HD void pass3(float2 (&u)[32])
 {
 #pragma unroll
@@ -166,6 +182,44 @@ DM_HD void x1_read(float2 (&u)[32], int rho, int t, const unsigned char *wbuf)
 {
     const int h = (t >> 4) ^ rho;                   // which register half this lane receives
     const unsigned char *p = wbuf + (t >> 4) * X1_BLK + (t & 15) * X1_ROW;
+    if (h == 0) {
+#pragma unroll
+        for (int b = 0; b < 16; b += 2) {
+            const float4 v = *reinterpret_cast<const float4 *>(p + b * 8);
+            u[b] = make_float2(v.x, v.y);
+            u[b + 1] = make_float2(v.z, v.w);
+        }
+    } else {
+#pragma unroll
+        for (int b = 0; b < 16; b += 2) {
+            const float4 v = *reinterpret_cast<const float4 *>(p + b * 8);
+            u[16 + b] = make_float2(v.x, v.y);
+            u[16 + b + 1] = make_float2(v.z, v.w);
+        }
+    }
+}
+
+// the same exchange with the rows of a warp split over `mainp` (rows 0..27) and `spare` (rows 28..31)
+DM_HD unsigned char *x1s_row(int r, unsigned char *mainp, unsigned char *spare)
+{
+    return r < X1S_MAIN_ROWS ? mainp + r * X1_ROW : spare + (r - X1S_MAIN_ROWS) * X1_ROW;
+}
+DM_HD void x1s_write(const float2 (&u)[32], int rho, int t, unsigned char *mainp, unsigned char *spare)
+{
+    const int h = (t >> 4) ^ rho;
+    const int col = (t & 15) * 8;
+    if (h == 0) {
+#pragma unroll
+        for (int j = 0; j < 16; ++j) *reinterpret_cast<float2 *>(mainp + j * X1_ROW + col) = u[j];
+    } else {
+#pragma unroll
+        for (int j = 0; j < 16; ++j) *reinterpret_cast<float2 *>(x1s_row(16 + j, mainp, spare) + col) = u[16 + j];
+    }
+}
+DM_HD void x1s_read(float2 (&u)[32], int rho, int t, unsigned char *mainp, unsigned char *spare)
+{
+    const int h = (t >> 4) ^ rho;
+    const unsigned char *p = x1s_row(t, mainp, spare);
     if (h == 0) {
 #pragma unroll
         for (int b = 0; b < 16; b += 2) {
@@ -257,7 +311,7 @@ struct RegArgs {
 //   half B (64 KiB): rows 64..127 of the next frame's psi
 // so the HBM time of a frame hides behind the FFTs of the previous / current frame.
 constexpr int PBUF_BYTES = 2 * 65536;
-constexpr int REG_SMEM_V1 = PBUF_BYTES + XBUF_BYTES + 2048;
+constexpr int REG_SMEM_V1 = PBUF_BYTES + XBUF3_BYTES + 2048;
 
 __device__ __forceinline__ float abs2_rn(float2 f) { return __fmaf_rn(f.y, f.y, __fmul_rn(f.x, f.x)); }
 
@@ -330,9 +384,10 @@ __global__ void __launch_bounds__(RNT, 1) regfft128_kernel(const RegArgs a)
     extern __shared__ __align__(16) unsigned char smem[];
     unsigned char *pbuf = smem;
     unsigned char *xbuf = smem + PBUF_BYTES;
-    float2 *s_wy = reinterpret_cast<float2 *>(smem + PBUF_BYTES + XBUF_BYTES);
+    float2 *s_wy = reinterpret_cast<float2 *>(smem + PBUF_BYTES + XBUF3_BYTES);
     float2 *s_wx = s_wy + 128;
     __shared__ float red[4 * 32];
+    __shared__ int s_rdcnt;                                     // warps that have finished reading the prefetch buffer in S1
     __shared__ uint32_t s_tmem;
     __shared__ __align__(8) uint64_t mb_lo, mb_hi, mb_amp;      // psi rows 0..63 (half A), rows 64..127 (half B), sqrt(I) (half A)
 
@@ -343,6 +398,7 @@ __global__ void __launch_bounds__(RNT, 1) regfft128_kernel(const RegArgs a)
     if (tid < 128) s_wy[tid] = a.wy[tid];
     else if (tid < 256) s_wx[tid - 128] = a.wx[tid - 128];
     if (tid == 0) {
+        s_rdcnt = 0;
         mbar_init(&mb_lo, 1);
         mbar_init(&mb_hi, 1);
         mbar_init(&mb_amp, 1);
@@ -360,7 +416,7 @@ __global__ void __launch_bounds__(RNT, 1) regfft128_kernel(const RegArgs a)
     const uint32_t t_psi = s_tmem + ((uint32_t)(32 * (w & 3)) << 16) + (uint32_t)(w >> 2) * 128u;
     const uint32_t t_po = t_psi + 64u;
 
-    unsigned char *wbuf = xbuf + w * X1_WARP;
+    unsigned char *wbuf = xbuf + w * 4096, *wspare = xbuf + X1S_SPARE_OFF + w * X1S_SPARE;
     float2 *xb2 = reinterpret_cast<float2 *>(xbuf);
     const float2 *Pk = a.P + (size_t)k * RNN + w * RN + t;
     const float cfac = a.beta > 0.f ? 1.f / (float)RNN : 0.f;
@@ -417,12 +473,16 @@ __global__ void __launch_bounds__(RNT, 1) regfft128_kernel(const RegArgs a)
                 }
             }
         }
-        __syncthreads();                    // the whole prefetch buffer has been read
-        RPROF(0)
-        if (tid == 0) {
+        // the warp that finishes reading the prefetch buffer LAST refills it; nobody waits (a block barrier here would
+        // hold the warps whose P and O arrived early back from their first FFT pass)
+        __syncwarp();
+        if (t == 0 && atomicAdd(&s_rdcnt, 1) == 15) {
+            s_rdcnt = 0;
+            asm volatile("fence.proxy.async.shared::cta;\n" ::: "memory");
             bulk_load(pbuf, a.amp + (size_t)view * RNN, 65536, &mb_amp);
             if (nview < a.n_views) bulk_load(pbuf + 65536, nsrc + 65536, 65536, &mb_hi);
         }
+        RPROF(0)
         tmem_wait_st();
         // ---- S3: forward 2-D FFT ----
         {
@@ -435,20 +495,36 @@ __global__ void __launch_bounds__(RNT, 1) regfft128_kernel(const RegArgs a)
         }
 #pragma unroll
         for (int rho = 0; rho < 2; ++rho) {
-            x1_write(u, rho, t, wbuf);
+            x1s_write(u, rho, t, wbuf, wspare);
             __syncwarp();
-            x1_read(u, rho, t, wbuf);
+            x1s_read(u, rho, t, wbuf, wspare);
             __syncwarp();
         }
         pass2<false>(u);
+        // exchange 2 in two rounds; M <= 2: the first half of pass 3 runs while the stores of the second round drain
+        // (c1 -2 %; with the larger S4 code of M >= 3 the reordering costs spills: c2 +1.3 %, so not there)
+        constexpr bool SPLIT3 = (MT == 1 || MT == 2);
+        if (SPLIT3) {
+            __syncthreads();
+            x2_write(u, 0, w, t, xb2);
+            __syncthreads();
+            x2_read(u, 0, w, t, xb2);
+            __syncthreads();
+            x2_write(u, 1, w, t, xb2);
+            pass3_half<false>(u, 0);
+            __syncthreads();
+            x2_read(u, 1, w, t, xb2);
+            pass3_half<false>(u, 1);
+        } else {
 #pragma unroll
-        for (int z = 0; z < 2; ++z) {
-            __syncthreads();
-            x2_write(u, z, w, t, xb2);
-            __syncthreads();
-            x2_read(u, z, w, t, xb2);
+            for (int z = 0; z < 2; ++z) {
+                __syncthreads();
+                x2_write(u, z, w, t, xb2);
+                __syncthreads();
+                x2_read(u, z, w, t, xb2);
+            }
+            pass3<false>(u);
         }
-        pass3<false>(u);
         RPROF(1)
         // ---- S4: mode-summed modulus constraint (|F|^2 exchanged through L2) ----
         {
@@ -524,23 +600,37 @@ __global__ void __launch_bounds__(RNT, 1) regfft128_kernel(const RegArgs a)
         }
         RPROF(3)
         // ---- S5: inverse 2-D FFT (mirror) ----
-        pass3<true>(u);
+        if (SPLIT3) {
+            pass3_half<true>(u, 0);
+            __syncthreads();
+            // every thread is past S4: half A (sqrt(I)) is free for the next frame's rows 0..63
+            if (tid == 0 && nview < a.n_views) bulk_load(pbuf, nsrc, 65536, &mb_lo);
+            x2_write(u, 0, w, t, xb2);
+            pass3_half<true>(u, 1);             // while the stores of round 0 drain
+            __syncthreads();
+            x2_read(u, 0, w, t, xb2);
+            __syncthreads();
+            x2_write(u, 1, w, t, xb2);
+            __syncthreads();
+            x2_read(u, 1, w, t, xb2);
+        } else {
+            pass3<true>(u);
 #pragma unroll
-        for (int z = 0; z < 2; ++z) {
-            __syncthreads();
-            // (z == 0) every thread is past S4: half A (sqrt(I)) is free for the next frame's rows 0..63
-            if (z == 0 && tid == 0 && nview < a.n_views) bulk_load(pbuf, nsrc, 65536, &mb_lo);
-            x2_write(u, z, w, t, xb2);
-            __syncthreads();
-            x2_read(u, z, w, t, xb2);
+            for (int z = 0; z < 2; ++z) {
+                __syncthreads();
+                if (z == 0 && tid == 0 && nview < a.n_views) bulk_load(pbuf, nsrc, 65536, &mb_lo);
+                x2_write(u, z, w, t, xb2);
+                __syncthreads();
+                x2_read(u, z, w, t, xb2);
+            }
         }
         pass2<true>(u);
-        __syncthreads();
+        // no block barrier: exchange 1 only touches what this warp itself read in exchange 2 and its spare strip
 #pragma unroll
         for (int rho = 0; rho < 2; ++rho) {
-            x1_write(u, rho, t, wbuf);
+            x1s_write(u, rho, t, wbuf, wspare);
             __syncwarp();
-            x1_read(u, rho, t, wbuf);
+            x1s_read(u, rho, t, wbuf, wspare);
             __syncwarp();
         }
         {
