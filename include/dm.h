@@ -213,6 +213,39 @@ dm_status dm_host_fft2(int N, const float *in_host, float *out_host, int inverse
  * for path 3 (UNSUPPORTED otherwise).                                                    */
 dm_status dm_host_fft2_path(int N, int path, const float *in_host, float *out_host, int inverse);
 
+/* Probe update without a workspace and without any allocation: eq. (5), PAPER.md:58,
+ *   P_k(r) = (alpha P_old_k(r) + sum_j sum_l conj(O_l(r + r_j)) psi_jkl(r)) / (alpha + sum_j sum_l |O_l(r + r_j)|^2),
+ * the same two-stage reduction dm_iterate runs as its step S8 (FP32 partial sums over contiguous view
+ * chunks, j ascending and l ascending inside; chunk-ascending FP64 second stage; P_new = P_old where the
+ * denominator is 0), for a caller that holds psi, O and P itself.
+ * For whom: every other call of this header needs a workspace the caller allocates.  A caller that may not
+ * allocate -- a plug-in in an application whose own pool took all device memory at start-up, a measurement-time
+ * loop in which cudaMalloc / cudaFree are forbidden because they stall every stream of the device and may fail
+ * -- has nowhere to put the partial sums.  Here they go into a fixed array of DM_NOALLOC_SCRATCH_BYTES that is
+ * part of the library image: the CUDA driver places it on each GPU that loads the library and keeps it until the
+ * process exits.  The call itself performs no cudaMalloc / cudaFree and uses no allocating library routine.
+ *   positions_dev  DEV int32 [n_views][2] = (y0, x0); NOT validated (they are device data): every window must
+ *                  lie inside the object, as dm_plan_create would have checked
+ *   object_dev     DEV c64 [L][obj_h][obj_w]        psi_dev  DEV c64 [n_views][K][L][N][N], 16-byte aligned
+ *   probe_old_dev  DEV c64 [K][N][N]                probe_new_dev  DEV c64 [K][N][N] (out; must not alias probe_old_dev)
+ *   alpha_probe    the ABSOLUTE regulariser (>= 0), e.g. dm_get_alphas()[1] of a plan, or 0 for the literal quotient
+ *   err_text_host  HOST char[err_text_bytes] or NULL: receives the text of a non-OK status (there is no plan to ask)
+ * Limit: N * N * (8 K + 4) bytes (one chunk of partial sums) must fit the array, else DM_ERR_WORKSPACE with both
+ * sizes in the text; within the limit, fewer chunks fit for larger N * N * K, which costs parallelism, not
+ * correctness (the FP32 summation order, hence the last bits, follows the chunk count).  Other errors:
+ * INVALID_ARG (null, sizes < 1, alpha < 0), UNSUPPORTED (N, K * L > 8), OUT_OF_BOUNDS (object smaller than a
+ * window), CUDA.  Async on `stream`.
+ * First call on each device: looks up the device address of the array (cudaGetSymbolAddress, once per device,
+ * with that device current) and the SM count; make that call outside any stream capture.
+ * Sharing: all calls on a device use the same array, which keeps the previous call's contents (nothing in it
+ * needs clearing: a call overwrites every slot it later reads).  Calls that overlap on the GPU (two streams,
+ * two host threads) race on it: serialise them.                                                              */
+#define DM_NOALLOC_SCRATCH_BYTES (16u << 20)
+dm_status dm_probe_update_noalloc(int N, int n_views, int K, int L, int obj_h, int obj_w,
+                                  const int32_t *positions_dev, const float *object_dev, const float *psi_dev,
+                                  const float *probe_old_dev, float alpha_probe, float *probe_new_dev, void *stream,
+                                  char *err_text_host, size_t err_text_bytes);
+
 const char *dm_status_string(dm_status s);
 const char *dm_last_error(const dm_plan *plan); /* plan may be NULL: last create error */
 void dm_plan_destroy(dm_plan *plan);

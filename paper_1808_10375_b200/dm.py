@@ -24,7 +24,8 @@ SYMBOLS = (
     "dm_plan_create", "dm_plan_set_param", "dm_plan_workspace_bytes", "dm_plan_set_workspace",
     "dm_set_data", "dm_iterate", "dm_get_probe", "dm_get_object", "dm_get_psi", "dm_get_errors",
     "dm_set_state", "dm_get_window_table", "dm_get_coverage", "dm_get_alphas", "dm_get_mode_power", "dm_solve_host",
-    "dm_plan_info", "dm_plan_geometry", "dm_plan_set_profiling", "dm_get_phase_ms", "dm_measure_peaks", "dm_host_fft2", "dm_host_fft2_path", "dm_status_string", "dm_last_error", "dm_plan_destroy",
+    "dm_plan_info", "dm_plan_geometry", "dm_plan_set_profiling", "dm_get_phase_ms", "dm_measure_peaks", "dm_host_fft2", "dm_host_fft2_path",
+    "dm_probe_update_noalloc", "dm_status_string", "dm_last_error", "dm_plan_destroy",
 )
 
 _vp, _int, _dbl = C.c_void_p, C.c_int, C.c_double
@@ -68,6 +69,7 @@ def lib() -> C.CDLL:
         L.dm_measure_peaks.argtypes = [_vp, C.c_size_t, _vp, _int, _vp]
         L.dm_host_fft2.argtypes = [_int, _vp, _vp, _int]
         L.dm_host_fft2_path.argtypes = [_int, _int, _vp, _vp, _int]
+        L.dm_probe_update_noalloc.argtypes = [_int] * 6 + [_vp] * 4 + [C.c_float, _vp, _vp, C.c_char_p, C.c_size_t]
         L.dm_status_string.argtypes = [_int]
         L.dm_status_string.restype = C.c_char_p
         L.dm_last_error.argtypes = [_vp]
@@ -110,6 +112,35 @@ def host_fft2(x: np.ndarray, inverse: bool = False, path: int = 0) -> np.ndarray
         st = lib().dm_host_fft2(x.shape[-1], _np_ptr(x), _np_ptr(out), int(inverse))
     if st != DM_OK:
         raise DMError(st, "dm_host_fft2")
+    return out
+
+
+NOALLOC_SCRATCH_BYTES = 16 << 20
+
+
+def probe_update_noalloc(positions, object_, psi, probe_old, alpha_probe, out=None, stream=None):
+    """dm_probe_update_noalloc: eq. (5) on device tensors the caller already holds, for callers that
+    cannot allocate device memory (an application whose pool owns the whole card, a loop where cudaMalloc's
+    device-wide stall is not acceptable): the partial sums go to a fixed NOALLOC_SCRATCH_BYTES array inside the
+    library instead of a workspace.  positions int32 [n_views][2] (device), object_ c64 [L][H][W], psi c64
+    [n_views][K][L][N][N], probe_old c64 [K][N][N]; returns P_new (written into `out` when given, so that this
+    wrapper allocates nothing either).  Calls share the array: do not overlap two of them on one GPU.  The first
+    call on a device does a one-time address look-up; keep it outside stream capture."""
+    import torch
+    n_views, K, L, N = psi.shape[0], psi.shape[1], psi.shape[2], psi.shape[-1]
+    H, W = object_.shape[-2:]
+    assert positions.is_cuda and positions.dtype == torch.int32 and positions.is_contiguous() and tuple(positions.shape) == (n_views, 2)
+    for t, shape in ((object_, (L, H, W)), (psi, (n_views, K, L, N, N)), (probe_old, (K, N, N))):
+        assert t.is_cuda and t.dtype == torch.complex64 and t.is_contiguous() and tuple(t.shape) == shape
+    if out is None:
+        out = torch.empty_like(probe_old)
+    assert out.is_cuda and out.dtype == torch.complex64 and out.is_contiguous() and tuple(out.shape) == (K, N, N)
+    err = C.create_string_buffer(512)
+    st = lib().dm_probe_update_noalloc(N, n_views, K, L, H, W, _vp(positions.data_ptr()), _vp(object_.data_ptr()),
+                                       _vp(psi.data_ptr()), _vp(probe_old.data_ptr()), float(alpha_probe),
+                                       _vp(out.data_ptr()), DMPlan._stream(stream), err, len(err))
+    if st != DM_OK:
+        raise DMError(st, err.value.decode())
     return out
 
 
