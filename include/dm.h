@@ -60,10 +60,7 @@ typedef enum {
                                  dm_set_data if N > 128), 3 = force the register-resident
                                  path (DM_ERR_UNSUPPORTED at dm_set_data unless N = 128),
                                  4 = force the view-pipelined warp-FFT path (any N; the
-                                 default for N >= 256), 5 = force the register-resident
-                                 path on clusters of two 256-thread CTAs, two CTAs per SM
-                                 (N = 128 only; measured slower than path 3, kept as the
-                                 record of that experiment)                   */
+                                 default for N >= 256)                                       */
     DM_PARAM_LAG = 5,         /* path 4: views between the row, column and inverse-row phases
                                  of one view (integer >= 1; 0 = derive from the task counts,
                                  default).  Sizes the scratch ring: set before
@@ -164,7 +161,7 @@ dm_status dm_solve_host(dm_plan *plan, const float *intensities_host, const floa
                         float *out_object_host, void *stream);
 
 /* Which path dm_iterate runs for this plan: 1 staged, 2 fused, 3 register-resident,
- * 4 view-pipelined warp-FFT, 5 register-resident on CTA pairs, 64 FP64 validation mode
+ * 4 view-pipelined warp-FFT, 64 FP64 validation mode
  * (valid after dm_set_data);
  * and how many kernels one iteration launches (the bench's gpu_launches claim).           */
 dm_status dm_plan_info(const dm_plan *plan, int *path, int *launches_per_iter);
@@ -175,7 +172,7 @@ dm_status dm_plan_info(const dm_plan *plan, int *path, int *launches_per_iter);
  *   [0] psi-update path (as dm_plan_info)      [1] SM count the grids were sized for
  *   [2] probe update (eq. (5)): CTAs along the view axis   [3] views summed by each of them
  *   [4] object update (eq. (6)): longest coverage list     [5] list entries per batch
- *   [6] paths 3, 5: persistent CTAs   [7] CTAs per view   [8] most views one of their groups takes
+ *   [6] path 3: persistent CTAs   [7] CTAs per view   [8] most views one of their groups takes
  *   [9] path 4: scratch ring slots    [10] phase lag (views)   [11] persistent CTAs   [12] warps per CTA
  *   [13] path 3: 1 = the CTAs of a view meet at a software barrier in L2, 0 = hardware cluster
  * [6]-[8], [11] and [13] are valid after dm_set_data (they come from occupancy queries).          */

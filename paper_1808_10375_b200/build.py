@@ -43,7 +43,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
     if not force and up_to_date():
         return LIB
     nvcc = os.environ.get("NVCC", "nvcc")
-    # DM_NVCC_EXTRA: extra nvcc flags (e.g. -DDM_PAIR_PROF, the clock64 phase profile of dm_pairfft.cuh)
+    # DM_NVCC_EXTRA: extra nvcc flags (e.g. -DDM_REG_PROF, the clock64 phase profile of dm_regfft.cuh)
     cmd = [nvcc] + NVCC_FLAGS + os.environ.get("DM_NVCC_EXTRA", "").split() + sources() + ["-o", LIB + ".tmp"]
     res = subprocess.run(cmd, stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True)
     log = os.path.join(HERE, "build.log")

@@ -11,7 +11,6 @@
 
 #include "../../include/dm.h"
 #include "dm_kernels.cuh"
-#include "dm_pairfft.cuh"
 #include "dm_fp64.cuh"
 
 namespace {
@@ -40,8 +39,8 @@ struct dm_plan {
     int path_req, path;                  // requested / chosen (1 staged, 2 fused, 3 register-resident)
     int reg_grid;                        // path 3: number of persistent CTAs (multiple of M)
     bool reg_sw;                         // path 3: software group barrier instead of a hardware cluster
-    int *reg_gbar;                       // paths 3, 5: [reg_cap] group barrier counters + 1 sticky "a CTA gave up waiting" flag (path 5)
-    int reg_cap;                         // paths 3, 5: upper bound on resident CTAs (2 per SM)
+    int *reg_gbar;                       // path 3: [reg_cap] group barrier counters (+ 1 spare word)
+    int reg_cap;                         // path 3: upper bound on resident CTAs (2 per SM)
     // path 4 (dm_warpfft.cuh): ring slots, phase lag (views), tasks per view and phase, persistent CTAs
     int wf_S, wf_D, wf_nA, wf_nB, wf_nC, wf_grid, wf_nw;
     int wf_lag_req;                      // 0 = derive the lag from the task counts
@@ -385,74 +384,6 @@ dm_status launch_regfft(dm_plan *plan, cudaStream_t st, bool query_only)
     }
 }
 
-// path 5: the register-resident transform on clusters of two 256-thread CTAs, two CTAs per SM (dm_pairfft.cuh)
-template <int MT> dm_status launch_pairfft_t(dm_plan *plan, cudaStream_t st, bool query_only)
-{
-    auto kern = dmpair::pairfft128_kernel<MT>;
-    if (query_only) CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, dmpair::PAIR_SMEM));
-    if (query_only) CU(cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));   // two CTAs per SM
-    cudaLaunchConfig_t cfg;
-    memset(&cfg, 0, sizeof cfg);
-    cfg.blockDim = dim3(dmpair::PNT);
-    cfg.dynamicSmemBytes = dmpair::PAIR_SMEM;
-    cfg.stream = st;
-    cudaLaunchAttribute at[1];
-    at[0].id = cudaLaunchAttributeClusterDimension;
-    at[0].val.clusterDim.x = 2;
-    at[0].val.clusterDim.y = 1;
-    at[0].val.clusterDim.z = 1;
-    cfg.attrs = at;
-    cfg.numAttrs = 1;
-    if (query_only) {
-        // Every CTA of the grid must be resident (the frames of a view wait on one another).  The occupancy API
-        // reports ONE block per SM for any kernel that allocates tensor memory (measured: even 32 columns),
-        // although the hardware co-schedules CTAs whose columns fit (4 x 128 columns run as one wave), so the
-        // two-CTAs-per-SM residency is derived here from the device limits themselves; a CTA that nevertheless
-        // waits too long at the group barrier gives up (dmpair::SPIN_LIMIT) instead of hanging.
-        int dev = 0, sms = 0, smem_sm = 0, regs_sm = 0;
-        cudaFuncAttributes fa;
-        CU(cudaGetDevice(&dev));
-        CU(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
-        CU(cudaDeviceGetAttribute(&smem_sm, cudaDevAttrMaxSharedMemoryPerMultiprocessor, dev));
-        CU(cudaDeviceGetAttribute(&regs_sm, cudaDevAttrMaxRegistersPerMultiprocessor, dev));
-        CU(cudaFuncGetAttributes(&fa, kern));
-        const size_t smem_cta = (size_t)dmpair::PAIR_SMEM + fa.sharedSizeBytes + 1024;
-        int per = 2;                                                // 2 x 256 tensor-memory columns
-        if ((size_t)per * smem_cta > (size_t)smem_sm) per = (int)((size_t)smem_sm / smem_cta);
-        if (per * fa.numRegs * dmpair::PNT > regs_sm) per = regs_sm / (fa.numRegs * dmpair::PNT);
-        int slots = sms * per / 2;
-        if (2 * slots > plan->reg_cap) slots = plan->reg_cap / 2;
-        int groups = slots / plan->M;
-        if (groups < 1) return fail(plan, DM_ERR_UNSUPPORTED, "pair kernel: %d clusters fit the device, a view needs %d", slots, plan->M);
-        if (groups > plan->n_views) groups = plan->n_views;
-        plan->reg_grid = 2 * groups * plan->M;
-        plan->reg_sw = plan->M > 1;
-        return DM_OK;
-    }
-    dmpair::PairArgs a;
-    memset(&a, 0, sizeof a);
-    a.n_views = plan->n_views; a.K = plan->K; a.L = plan->L; a.H = plan->H; a.W = plan->W;
-    a.pos = plan->pos_d; a.P = plan->Pbuf[plan->curP]; a.O = plan->Obuf[plan->curO];
-    a.psi = plan->psi; a.amp = plan->amp; a.wy = plan->wy_d; a.wx = plan->wx_d;
-    a.sbuf = plan->sbuf; a.part = plan->partA; a.gbar = plan->reg_gbar; a.gave_up = plan->reg_gbar + plan->reg_cap;
-    a.beta = (float)plan->beta; a.eps = (float)plan->eps_f;
-    cfg.gridDim = dim3((unsigned)plan->reg_grid);
-    if (plan->M > 1) CU(cudaMemsetAsync(plan->reg_gbar, 0, (size_t)plan->reg_cap * sizeof(int), st));
-    CU(cudaLaunchKernelEx(&cfg, kern, a));
-    return DM_OK;
-}
-
-dm_status launch_pairfft(dm_plan *plan, cudaStream_t st, bool query_only)
-{
-    switch (plan->M) {
-    case 1: return launch_pairfft_t<1>(plan, st, query_only);
-    case 2: return launch_pairfft_t<2>(plan, st, query_only);
-    case 3: return launch_pairfft_t<3>(plan, st, query_only);
-    case 4: return launch_pairfft_t<4>(plan, st, query_only);
-    default: return launch_pairfft_t<0>(plan, st, query_only);
-    }
-}
-
 // path 4: persistent task-queue kernel (rows -> columns + modulus -> rows through an L2-resident ring)
 template <int N> dm_status launch_wf_t(dm_plan *plan, cudaStream_t st, bool query_only)
 {
@@ -502,7 +433,6 @@ dm_status launch_psi_update(dm_plan *plan, cudaStream_t st, bool prepare = false
 {
     if (plan->path == 4) return launch_wf(plan, st, prepare);
     if (plan->path == 3) return launch_regfft(plan, st, prepare);
-    if (plan->path == 5) return launch_pairfft(plan, st, prepare);
     if (plan->path == 2) {
         if (plan->N == 64) return launch_fused<64, 256>(plan, st, prepare);
         return launch_fused<128, 512>(plan, st, prepare);
@@ -646,7 +576,7 @@ dm_status dm_plan_set_param(dm_plan *plan, dm_param which, double v)
     case DM_PARAM_ALPHA_OBJ: if (v < 0) break; plan->a_obj = v; return DM_OK;
     case DM_PARAM_ALPHA_PROBE: if (v < 0) break; plan->a_probe = v; return DM_OK;
     case DM_PARAM_EPS_F: if (v < 0) break; plan->eps_f = v; return DM_OK;
-    case DM_PARAM_PATH: if (v != 0 && v != 1 && v != 2 && v != 3 && v != 4 && v != 5) break; plan->path_req = (int)v; return DM_OK;
+    case DM_PARAM_PATH: if (v != 0 && v != 1 && v != 2 && v != 3 && v != 4) break; plan->path_req = (int)v; return DM_OK;
     case DM_PARAM_PRECISION:
         if (v != 0 && v != 1) break;
         if (plan->ws) return fail(plan, DM_ERR_INVALID_ARG, "the precision sizes the workspace: set it before dm_plan_set_workspace");
@@ -805,8 +735,8 @@ dm_status set_data_impl(dm_plan *plan, const float *intensities, const float *pr
     if (plan->precision == 1) path = 64;         // FP64 validation mode: its own plain kernels
     if (path == 2 && plan->N > 128)
         return fail(plan, DM_ERR_UNSUPPORTED, "fused per-frame path needs N <= 128 (N = %d)", plan->N);
-    if ((path == 3 || path == 5) && plan->N != 128)
-        return fail(plan, DM_ERR_UNSUPPORTED, "register-resident paths need N = 128 (N = %d)", plan->N);
+    if (path == 3 && plan->N != 128)
+        return fail(plan, DM_ERR_UNSUPPORTED, "register-resident path needs N = 128 (N = %d)", plan->N);
     plan->path = path;
     cudaStream_t st = (cudaStream_t)stream;
     const size_t NN = (size_t)plan->N * plan->N, HW = (size_t)plan->H * plan->W;
@@ -815,7 +745,7 @@ dm_status set_data_impl(dm_plan *plan, const float *intensities, const float *pr
     // intensities of dm_solve_host on the copy engine)
     if (plan->tables_path != path) {
     plan->spec.assign(NN, 0);
-    if (path == 3 || path == 5) {
+    if (path == 3) {
         for (int tid = 0; tid < dmreg::RNT; ++tid)
             for (int e = 0; e < dmreg::REPT; ++e) plan->spec[dmreg::spec_pos(tid, e)] = dmreg::spec_freq(tid, e);
         std::vector<float> wy(256), wx(256);
@@ -886,7 +816,6 @@ dm_status set_data_impl(dm_plan *plan, const float *intensities, const float *pr
     CU(cudaMemcpyAsync(plan->Pbuf[0], probe0, plan->K * NN * sizeof(float2), cudaMemcpyDeviceToDevice, st));
     CU(cudaMemcpyAsync(plan->Obuf[0], object0, plan->L * HW * sizeof(float2), cudaMemcpyDeviceToDevice, st));
     CU(cudaMemsetAsync(plan->alphas, 0, 2 * sizeof(float), st));
-    CU(cudaMemsetAsync(plan->reg_gbar + plan->reg_cap, 0, sizeof(int), st));
     const size_t total = (size_t)plan->n_views * NN;
     if (n_chunks <= 0) amp_permute_kernel<<<plan->sms * 8, 256, 0, st>>>(plan->N, intensities, plan->spec_d, plan->amp, total);
     psi_init_kernel<<<dim3((unsigned)((NN + 1023) / 1024), (unsigned)(plan->n_views * plan->M)), 256, 0, st>>>(
@@ -961,7 +890,7 @@ dm_status dm_iterate(dm_plan *plan, int n_iter, void *stream)
         if (plan->path == 4) {
             e.pF = plan->partA; e.nF = plan->n_views * plan->wf_nB; e.sF = 2;
             e.pS = plan->partB; e.nS = plan->n_views * plan->wf_nC; e.sS = 2;
-        } else if (plan->path == 3 || plan->path == 5) {
+        } else if (plan->path == 3) {
             e.pF = plan->partA;     e.nF = plan->reg_grid; e.sF = 4;
             e.pS = plan->partA + 2; e.nS = plan->reg_grid; e.sS = 4;
         } else if (plan->path == 2) {
@@ -1039,11 +968,6 @@ dm_status dm_get_errors(const dm_plan *plan, double *out_host, int max_rows, int
     if (s != DM_OK) return s;
     if (!out_host || !rows_written || max_rows < 0) return fail(plan, DM_ERR_INVALID_ARG, "bad output arguments");
     CU(cudaDeviceSynchronize());
-    if (plan->path == 5) {      // the pair kernel's CTAs wait on one another; one that gave up (grid not resident) leaves garbage
-        int gave_up = 0;
-        CU(cudaMemcpy(&gave_up, plan->reg_gbar + plan->reg_cap, sizeof(int), cudaMemcpyDeviceToHost));
-        if (gave_up) return fail(plan, DM_ERR_CUDA, "path 5: a CTA timed out at the group barrier (its grid was not resident); results are invalid");
-    }
     const int n = plan->rows < max_rows ? plan->rows : max_rows;
     if (n > 0) CU(cudaMemcpy(out_host, plan->errors, (size_t)n * (2 + plan->K + plan->L) * sizeof(double), cudaMemcpyDeviceToHost));
     *rows_written = n;
@@ -1222,8 +1146,8 @@ dm_status dm_plan_geometry(const dm_plan *plan, int32_t *out_host, int n_out)
     if (!plan || !out_host || n_out < 0) return DM_ERR_INVALID_ARG;
     int path = 0;
     dm_plan_info(plan, &path, nullptr);
-    const bool reg = path == 3 || path == 5;
-    const int per_view = path == 5 ? 2 * plan->M : plan->M;
+    const bool reg = path == 3;
+    const int per_view = plan->M;
     const int clusters = reg && plan->reg_grid > 0 ? plan->reg_grid / per_view : 0;
     const int32_t g[DM_GEOMETRY_FIELDS] = {
         path, plan->sms, plan->prb_chunks, plan->prb_chunk_len, plan->max_list, OBJ_NT,
@@ -1273,7 +1197,7 @@ void host_fft2_reg(const float *in, float *out, int inverse)
 {
     using namespace dmreg;
     std::vector<float2> regs((size_t)RNT * REPT);
-    std::vector<float4> xbuf_v(XBUF_BYTES / 16);
+    std::vector<float4> xbuf_v(XBUF3_BYTES / 16);      // the kernel's exchange buffer: 64 KiB + the 16 spare strips
     unsigned char *xbuf = reinterpret_cast<unsigned char *>(xbuf_v.data());
     std::vector<float2> wy(128), wx(128);
     for (int w = 0; w < 16; ++w)
@@ -1291,8 +1215,11 @@ void host_fft2_reg(const float *in, float *out, int inverse)
     float2 *dst = reinterpret_cast<float2 *>(out);
     auto exch1 = [&]() {
         for (int rho = 0; rho < 2; ++rho) {
-            for (int tid = 0; tid < RNT; ++tid) x1_write(U(tid), rho, tid & 31, xbuf + (tid >> 5) * X1_WARP);
-            for (int tid = 0; tid < RNT; ++tid) x1_read(U(tid), rho, tid & 31, xbuf + (tid >> 5) * X1_WARP);
+            // the kernel's own addressing: a warp's rows 0..27 inside its 4 KiB exchange-2 region, rows 28..31 in its spare strip
+            for (int tid = 0; tid < RNT; ++tid)
+                x1s_write(U(tid), rho, tid & 31, xbuf + (tid >> 5) * 4096, xbuf + X1S_SPARE_OFF + (tid >> 5) * X1S_SPARE);
+            for (int tid = 0; tid < RNT; ++tid)
+                x1s_read(U(tid), rho, tid & 31, xbuf + (tid >> 5) * 4096, xbuf + X1S_SPARE_OFF + (tid >> 5) * X1S_SPARE);
         }
     };
     auto exch2 = [&]() {

@@ -34,8 +34,7 @@ using namespace dmfft;
 
 constexpr int RN = 128, RNN = RN * RN, RNT = 512, REPT = 32;
 // exchange buffer: 16 warps x (2 blocks of 16 rows x 144 B) for exchange 1, 64 KiB for exchange 2
-constexpr int X1_ROW = 144, X1_BLK = 16 * X1_ROW, X1_WARP = 2 * X1_BLK;       // bytes
-constexpr int XBUF_BYTES = 16 * X1_WARP;                                       // 73728 >= 65536 (contiguous exchange-1 regions: path 5, host emulation)
+constexpr int X1_ROW = 144;                                                     // bytes
 // path 3 keeps a warp's exchange-1 rows inside the 4 KiB that the same warp reads in exchange 2 (rows 0..27) plus a
 // private spare strip behind the 64 KiB (rows 28..31), so exchange 1 never touches what another warp still has to
 // read: no block barrier between exchange 2 and exchange 1.  Spare strips start at 64 (mod 128) bytes: the 128-bit
@@ -164,42 +163,8 @@ template <bool INV> DM_HD void pass3(float2 (&u)[32])
 // Round rho moves the elements (reg a', lane b) with (a' >> 4) == (b >> 4) ^ rho, so every lane
 // writes 16 registers and reads 16 registers per round (4.5 KiB of buffer per warp).  Rows of
 // 16 elements are padded to 144 B: 64-bit stores of a row and 128-bit loads down a column
-// are both bank-conflict free.  wbuf = this warp's 4608-byte region.
-DM_HD void x1_write(const float2 (&u)[32], int rho, int t, unsigned char *wbuf)
-{
-    const int h = (t >> 4) ^ rho;                   // which register half this lane sends
-    unsigned char *p = wbuf + h * X1_BLK + (t & 15) * 8;
-    if (h == 0) {
-#pragma unroll
-        for (int j = 0; j < 16; ++j) *reinterpret_cast<float2 *>(p + j * X1_ROW) = u[j];
-    } else {
-#pragma unroll
-        for (int j = 0; j < 16; ++j) *reinterpret_cast<float2 *>(p + j * X1_ROW) = u[16 + j];
-    }
-}
-
-DM_HD void x1_read(float2 (&u)[32], int rho, int t, const unsigned char *wbuf)
-{
-    const int h = (t >> 4) ^ rho;                   // which register half this lane receives
-    const unsigned char *p = wbuf + (t >> 4) * X1_BLK + (t & 15) * X1_ROW;
-    if (h == 0) {
-#pragma unroll
-        for (int b = 0; b < 16; b += 2) {
-            const float4 v = *reinterpret_cast<const float4 *>(p + b * 8);
-            u[b] = make_float2(v.x, v.y);
-            u[b + 1] = make_float2(v.z, v.w);
-        }
-    } else {
-#pragma unroll
-        for (int b = 0; b < 16; b += 2) {
-            const float4 v = *reinterpret_cast<const float4 *>(p + b * 8);
-            u[16 + b] = make_float2(v.x, v.y);
-            u[16 + b + 1] = make_float2(v.z, v.w);
-        }
-    }
-}
-
-// the same exchange with the rows of a warp split over `mainp` (rows 0..27) and `spare` (rows 28..31)
+// are both bank-conflict free.  The 32 rows of a warp are split over `mainp` (rows 0..27, inside
+// the 4 KiB the warp itself reads in exchange 2) and `spare` (rows 28..31, its private strip).
 DM_HD unsigned char *x1s_row(int r, unsigned char *mainp, unsigned char *spare)
 {
     return r < X1S_MAIN_ROWS ? mainp + r * X1_ROW : spare + (r - X1S_MAIN_ROWS) * X1_ROW;
@@ -475,8 +440,12 @@ __global__ void __launch_bounds__(RNT, 1) regfft128_kernel(const RegArgs a)
         }
         // the warp that finishes reading the prefetch buffer LAST refills it; nobody waits (a block barrier here would
         // hold the warps whose P and O arrived early back from their first FFT pass)
+        // release / acquire around the counter: the other warps' reads of pbuf are ordered before the refill by the
+        // memory model (fence + atomic on both sides), not only by the data dependence of their tcgen05.st on the loads
         __syncwarp();
+        if (t == 0) __threadfence_block();
         if (t == 0 && atomicAdd(&s_rdcnt, 1) == 15) {
+            __threadfence_block();
             s_rdcnt = 0;
             asm volatile("fence.proxy.async.shared::cta;\n" ::: "memory");
             bulk_load(pbuf, a.amp + (size_t)view * RNN, 65536, &mb_amp);
@@ -626,6 +595,7 @@ __global__ void __launch_bounds__(RNT, 1) regfft128_kernel(const RegArgs a)
         }
         pass2<true>(u);
         // no block barrier: exchange 1 only touches what this warp itself read in exchange 2 and its spare strip
+        __syncwarp();           // every lane's exchange-2 reads of that region are done before any lane overwrites it
 #pragma unroll
         for (int rho = 0; rho < 2; ++rho) {
             x1s_write(u, rho, t, wbuf, wspare);

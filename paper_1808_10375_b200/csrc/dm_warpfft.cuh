@@ -10,7 +10,7 @@
 //   line of length N = 32 RX (RX = N/32 in {2,4,8,16});  a warp holds G = 32/RX lines;
 //   register a = g RX + r of lane t holds element n = t + 32 r of line g
 //   stage 1   radix-RX over r (-> k1), twiddle w_N^(t k1)
-//   exchange  (lane t, reg a) -> (lane a, reg t)                        [dmreg::x1_write/x1_read]
+//   exchange  (lane t, reg a) -> (lane a, reg t)                        [xt_write / xt_read below]   
 //   stage 2   radix-32 over t (-> k2):   frequency k = k1 + RX k2, held by lane a = g RX + k1
 //
 // Three phases per view, all running in ONE persistent kernel that pulls tasks from a queue in

@@ -107,15 +107,15 @@ def forced_pair(dm, pr, t_state, **params):
 
 
 @pytest.mark.parametrize("cfg_i,ny,nx", SMALL)
-@pytest.mark.parametrize("path", [0, 1, 2, 3, 4, 5])
+@pytest.mark.parametrize("path", [0, 1, 2, 3, 4])
 def test_one_iteration_parity(dm, cfg_i, ny, nx, path):
     """P2: set_data state (psi = P0*O0, frozen alphas) is exact; then one full iteration from an
     identical on-trajectory state (oracle state after 1 iteration) within 1e-5 on psi, P, O.
     path 0 = what dm_iterate picks (register-resident kernel for N = 128, fused shared-memory
-    kernel for N = 64, view-pipelined warp-FFT kernel above); 1, 2, 3, 4, 5 force the staged /
-    fused / register-resident / warp-FFT / CTA-pair register-resident path."""
+    kernel for N = 64, view-pipelined warp-FFT kernel above); 1, 2, 3, 4 force the staged /
+    fused / register-resident / warp-FFT path."""
     N = synth.CONFIGS[cfg_i].N
-    if (path == 2 and N > 128) or (path in (3, 5) and N != 128):
+    if (path == 2 and N > 128) or (path == 3 and N != 128):
         pytest.skip("path not defined for this frame size")
     if path == 1 and cfg_i not in (0, 3):
         pytest.skip("path 1 (the first, staged kernels; no configuration defaults to it) is kept as a cross-check on one "
@@ -350,20 +350,10 @@ def test_mid_size_one_step_reaches_full_size_loop_shapes(dm, cfg_i, ny, nx):
     assert geo["prb_chunk_len"] >= 5, geo
     if cfg_i in (2, 3):
         assert geo["obj_max_list"] > geo["obj_batch"], geo
-    if geo["path"] in (3, 5):
+    if geo["path"] == 3:
         assert geo["reg_views_per_group"] >= 3, geo
     if geo["path"] == 4:
         assert pr.cfg.n_views > geo["wf_slots"], geo
-
-
-@pytest.mark.parametrize("cfg_i,ny,nx", [(1, 20, 20), (2, 30, 30)])
-def test_mid_size_one_step_path5(dm, cfg_i, ny, nx):
-    """The same mid-size one-step comparison for the CTA-pair kernel (path 5): every cluster takes >= 3 views, so
-    its prefetch ring, the exchange-2 barrier parity and the group barrier counters all wrap."""
-    pr = synth.make_problem(synth.CONFIGS[cfg_i].scaled(ny, nx))
-    geo, r = _one_forced_step(dm, pr, f"cfg{cfg_i} {ny}x{nx} path 5", path=5)
-    print(f"cfg{cfg_i} {ny}x{nx} path 5: geometry {geo}; deviations {r}")
-    assert geo["path"] == 5 and geo["reg_views_per_group"] >= 3, geo
 
 
 @pytest.mark.parametrize("cfg_i", [1, 2])
@@ -384,13 +374,13 @@ def test_full_config_one_step(dm, cfg_i):
 @pytest.mark.parametrize("N,K,L,ny,nx", [(128, 4, 2, 3, 3), (128, 3, 1, 4, 3), (128, 1, 1, 5, 4), (128, 1, 5, 2, 3),
                                           (64, 2, 2, 4, 5), (64, 7, 1, 3, 2), (256, 1, 1, 2, 2), (256, 5, 1, 2, 2),
                                           (128, 2, 1, 1, 1)])
-@pytest.mark.parametrize("path", [0, 3, 4, 5])
+@pytest.mark.parametrize("path", [0, 3, 4])
 def test_mode_counts_and_ragged_shapes(dm, N, K, L, ny, nx, path):
     """Edge cases of the launch geometry: every compiled / run-time mode count M = K*L (1, 2, 3, 4,
     5, 7, 8), one single view, rasters that leave ragged last tiles / clusters / tasks; one iteration
     from the oracle's state after its first iteration, on every path defined for that N."""
     import dataclasses
-    if path in (3, 5) and N != 128:
+    if path == 3 and N != 128:
         pytest.skip("path not defined for this frame size")
     base = {64: synth.CONFIGS[0], 128: synth.CONFIGS[1], 256: synth.CONFIGS[3]}[N]
     w = tuple(np.linspace(1.0, 0.3, K) / np.linspace(1.0, 0.3, K).sum())
