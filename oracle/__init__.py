@@ -35,6 +35,17 @@ def lib(real: str = "f64") -> C.CDLL:
         L.oracle_object_update.restype = None
         L.oracle_probe_update.argtypes = [C.c_int] * 6 + [_vp] * 4 + [rt, _vp]
         L.oracle_probe_update.restype = None
+        L.oracle_views_update.argtypes = [C.c_int] * 5 + [_vp, _vp, C.c_int, C.c_int, _vp, _vp, _vp, rt, rt, _vp]
+        L.oracle_views_update.restype = None
+        for f in ("oracle_object_accumulate", "oracle_probe_accumulate"):
+            getattr(L, f).argtypes = [C.c_int] * 7 + [_vp] * 5
+            getattr(L, f).restype = None
+        L.oracle_object_finish.argtypes = [C.c_int] * 3 + [_vp] * 3 + [rt, _vp]
+        L.oracle_object_finish.restype = None
+        L.oracle_probe_finish.argtypes = [C.c_int] * 2 + [_vp] * 3 + [rt, _vp]
+        L.oracle_probe_finish.restype = None
+        L.oracle_frozen_alphas.argtypes = [C.c_int] * 6 + [_vp] * 3 + [rt, rt, _vp]
+        L.oracle_frozen_alphas.restype = None
         L.oracle_rel_change.argtypes = [C.c_size_t, _vp, _vp]
         L.oracle_rel_change.restype = rt
         L.oracle_create.argtypes = [C.c_int] * 6 + [_vp]
@@ -167,6 +178,72 @@ def probe_update(positions, O, psi, P_old, alpha=0.0, real="f64"):
     lib(real).oracle_probe_update(N, pos.shape[0], K, L, H, W, _p(pos), _p(O), _p(psi), _p(P_old),
                                   alpha, _p(out))
     return out
+
+
+# ---- view-range entry points: the same steps cut along the view axis (streaming of full-size problems) ----
+def views_update(positions, j0, j1, P, O, psi_range, amp_range, beta=1.0, eps=1e-30, real="f64"):
+    """Step A on views j0..j1-1 (oracle_view_update per view).  psi_range [j1-j0][K][L][N][N] ->
+    (psi_new_range, acc [j1-j0][4])."""
+    rt, ct = _types(real)
+    pos, P, O, amp = _c(positions, np.int32), _c(P, ct), _c(O, ct), _c(amp_range, rt)
+    psi = np.array(psi_range, dtype=ct, order="C", copy=True)
+    K, N = P.shape[0], P.shape[-1]
+    L, H, W = O.shape
+    assert psi.shape == (j1 - j0, K, L, N, N) and amp.shape == (j1 - j0, N, N) and 0 <= j0 <= j1 <= pos.shape[0]
+    acc = np.zeros((j1 - j0, 4), rt)
+    lib(real).oracle_views_update(N, j0, j1, K, L, _p(P), _p(O), H, W, _p(pos), _p(psi), _p(amp), beta, eps, _p(acc))
+    return psi, acc.astype(np.float64)
+
+
+def object_accumulate(positions, j0, j1, P, psi_range, num, den, real="f64"):
+    """eq. (6) sums of views j0..j1-1 added IN PLACE onto num (complex [L][H][W]) and den (real [H][W])."""
+    rt, ct = _types(real)
+    pos, P, psi = _c(positions, np.int32), _c(P, ct), _c(psi_range, ct)
+    K, N = P.shape[0], P.shape[-1]
+    L, H, W = num.shape
+    assert num.dtype == ct and den.dtype == rt and num.flags.c_contiguous and den.flags.c_contiguous and den.shape == (H, W)
+    assert psi.shape == (j1 - j0, K, L, N, N)
+    lib(real).oracle_object_accumulate(N, j0, j1, K, L, H, W, _p(pos), _p(P), _p(psi), _p(num), _p(den))
+
+
+def object_finish(num, den, O_old, alpha=0.0, real="f64"):
+    rt, ct = _types(real)
+    O_old = _c(O_old, ct)
+    L, H, W = O_old.shape
+    out = np.empty_like(O_old)
+    lib(real).oracle_object_finish(L, H, W, _p(_c(num, ct)), _p(_c(den, rt)), _p(O_old), alpha, _p(out))
+    return out
+
+
+def probe_accumulate(positions, j0, j1, O, psi_range, num, den, real="f64"):
+    """eq. (5) sums of views j0..j1-1 added IN PLACE onto num (complex [K][N][N]) and den (real [N][N])."""
+    rt, ct = _types(real)
+    pos, O, psi = _c(positions, np.int32), _c(O, ct), _c(psi_range, ct)
+    L, H, W = O.shape
+    K, N = num.shape[0], num.shape[-1]
+    assert num.dtype == ct and den.dtype == rt and num.flags.c_contiguous and den.flags.c_contiguous and den.shape == (N, N)
+    assert psi.shape == (j1 - j0, K, L, N, N)
+    lib(real).oracle_probe_accumulate(N, j0, j1, K, L, H, W, _p(pos), _p(O), _p(psi), _p(num), _p(den))
+
+
+def probe_finish(num, den, P_old, alpha=0.0, real="f64"):
+    rt, ct = _types(real)
+    P_old = _c(P_old, ct)
+    K, N = P_old.shape[0], P_old.shape[-1]
+    out = np.empty_like(P_old)
+    lib(real).oracle_probe_finish(N, K, _p(_c(num, ct)), _p(_c(den, rt)), _p(P_old), alpha, _p(out))
+    return out
+
+
+def frozen_alphas(positions, P0, O0, a_obj=1e-3, a_probe=1e-3, real="f64"):
+    """(alpha_obj, alpha_probe) as oracle_set_data freezes them (A8), without a state object."""
+    rt, ct = _types(real)
+    pos, P0, O0 = _c(positions, np.int32), _c(P0, ct), _c(O0, ct)
+    K, N = P0.shape[0], P0.shape[-1]
+    L, H, W = O0.shape
+    out = np.zeros(2)
+    lib(real).oracle_frozen_alphas(N, pos.shape[0], K, L, H, W, _p(pos), _p(P0), _p(O0), a_obj, a_probe, _p(out))
+    return tuple(out)
 
 
 def mode_power(modes):

@@ -19,7 +19,9 @@
  * projection idempotence and |F'|^2 sum == I; DM fixed point on noise-free data;
  * fused-form identity; overlap projection closed forms and least-squares property;
  * a dense-DFT-matrix numpy restatement of 3 whole iterations on a tiny case;
- * equivariances; tables against brute force.  Convergence magnitudes on config 0 are
+ * equivariances; tables against brute force; the view-range entry points at the end of
+ * this file (streaming of configs 3, 4) bit-identical to the monolithic steps for any split
+ * of the views and to oracle_iterate over two iterations.  Convergence magnitudes on config 0 are
  * reported only: "parity unpinned" versus any published number (the paper prints none).
  *
  * Build: gcc -O2 -fopenmp -shared -fPIC (see oracle/build.py).  -DORACLE_REAL=float
@@ -492,3 +494,148 @@ void oracle_set_num_threads(int n)
 #endif
 }
 int oracle_real_bytes(void) { return (int)sizeof(real); }
+
+/* ------------------------------------------------ view-range entry points ----
+ * The same steps as oracle_iterate, cut along the view axis so that a caller can stream a
+ * problem whose psi (complex128: 32 GiB for BASELINE.json config 3) does not fit host memory.
+ * Nothing new is computed: eq. (6) / eq. (5) are sums over the views j, and a sum
+ * carried in a caller-held accumulator over consecutive ranges [j0, j1) performs exactly the additions
+ * of oracle_object_update / oracle_probe_update in exactly their order (j ascending, then k resp. l
+ * ascending: readings A3, A15 of DESIGN.md), so the results are bit-identical to the monolithic
+ * functions for any split -- which tests/test_oracle_dm.py requires.  The denominators do not depend on
+ * the mode of the numerator (A15), so one [H][W] resp. [N][N] array serves all modes.              */
+
+/* Step A on views j0 <= j < j1 (each one oracle_view_update, as in oracle_iterate).
+ * psi_range_io [j1-j0][K][L][N][N] in/out, amp_range [j1-j0][N][N], acc_out [j1-j0][4].        */
+void oracle_views_update(int N, int j0, int j1, int K, int L, const real *P_in, const real *O_in,
+                         int obj_h, int obj_w, const int32_t *positions, real *psi_range_io,
+                         const real *amp_range, real beta, real eps, real *acc_out)
+{
+    size_t NN = (size_t)N * N;
+#pragma omp parallel for schedule(dynamic, 1)
+    for (int j = j0; j < j1; ++j) {
+        real a[4] = {0, 0, 0, 0};
+        oracle_view_update(N, K, L, P_in, O_in, obj_h, obj_w, positions[2 * j], positions[2 * j + 1],
+                           psi_range_io + 2 * (size_t)(j - j0) * K * L * NN,
+                           amp_range + (size_t)(j - j0) * NN, beta, eps, a, 0);
+        memcpy(acc_out + 4 * (size_t)(j - j0), a, sizeof(a));
+    }
+}
+
+/* eq. (6) numerator / denominator of views j0 <= j < j1 added onto num (cplx [L][H][W]) and den
+ * (real [H][W]); the caller zeroes both before the first range.  positions = the FULL list.     */
+void oracle_object_accumulate(int N, int j0, int j1, int K, int L, int obj_h, int obj_w,
+                              const int32_t *positions, const real *P_in, const real *psi_range_in,
+                              real *num_io, real *den_io)
+{
+    const cplx *P = (const cplx *)P_in, *psi = (const cplx *)psi_range_in;
+    cplx *numa = (cplx *)num_io;
+    size_t NN = (size_t)N * N, HW = (size_t)obj_h * obj_w;
+#pragma omp parallel for schedule(static)
+    for (int y = 0; y < obj_h; ++y)
+        for (int x = 0; x < obj_w; ++x)
+            for (int l = 0; l < L; ++l) {
+                size_t o = (size_t)y * obj_w + x;
+                cplx num = numa[l * HW + o]; real den = den_io[o];
+                for (int j = j0; j < j1; ++j) {
+                    int ry = y - positions[2 * j], rx = x - positions[2 * j + 1];
+                    if (ry < 0 || ry >= N || rx < 0 || rx >= N) continue;
+                    size_t r = (size_t)ry * N + rx;
+                    for (int k = 0; k < K; ++k) {
+                        cplx p = P[k * NN + r];
+                        num += conj(p) * psi[(((size_t)(j - j0) * K + k) * L + l) * NN + r];
+                        den += cabs2(p);
+                    }
+                }
+                numa[l * HW + o] = num;
+                if (l == L - 1) den_io[o] = den;    /* every l walks the same den sequence: store it once */
+            }
+}
+
+/* the quotient of eq. (6) with the inertial term (A8), as in oracle_object_update */
+void oracle_object_finish(int L, int obj_h, int obj_w, const real *num_in, const real *den_in,
+                          const real *O_old_in, real alpha, real *O_new_out)
+{
+    const cplx *num = (const cplx *)num_in, *Oo = (const cplx *)O_old_in;
+    cplx *On = (cplx *)O_new_out;
+    size_t HW = (size_t)obj_h * obj_w;
+    for (int l = 0; l < L; ++l)
+        for (size_t o = 0; o < HW; ++o) {
+            real den = den_in[o];
+            On[l * HW + o] = (alpha + den > 0) ? (alpha * Oo[l * HW + o] + num[l * HW + o]) / (alpha + den)
+                                               : Oo[l * HW + o];
+        }
+}
+
+/* eq. (5) numerator / denominator of views j0 <= j < j1 added onto num (cplx [K][N][N]) and den
+ * (real [N][N]); O is the NEW object (A3).                                                      */
+void oracle_probe_accumulate(int N, int j0, int j1, int K, int L, int obj_h, int obj_w,
+                             const int32_t *positions, const real *O_in, const real *psi_range_in,
+                             real *num_io, real *den_io)
+{
+    const cplx *O = (const cplx *)O_in, *psi = (const cplx *)psi_range_in;
+    cplx *numa = (cplx *)num_io;
+    size_t NN = (size_t)N * N, HW = (size_t)obj_h * obj_w;
+#pragma omp parallel for schedule(static)
+    for (int ry = 0; ry < N; ++ry)
+        for (int rx = 0; rx < N; ++rx)
+            for (int k = 0; k < K; ++k) {
+                size_t r = (size_t)ry * N + rx;
+                cplx num = numa[k * NN + r]; real den = den_io[r];
+                for (int j = j0; j < j1; ++j)
+                    for (int l = 0; l < L; ++l) {
+                        cplx o = O[l * HW + (size_t)(positions[2 * j] + ry) * obj_w +
+                                   positions[2 * j + 1] + rx];
+                        num += conj(o) * psi[(((size_t)(j - j0) * K + k) * L + l) * NN + r];
+                        den += cabs2(o);
+                    }
+                numa[k * NN + r] = num;
+                if (k == K - 1) den_io[r] = den;
+            }
+}
+
+void oracle_probe_finish(int N, int K, const real *num_in, const real *den_in, const real *P_old_in,
+                         real alpha, real *P_new_out)
+{
+    const cplx *num = (const cplx *)num_in, *Po = (const cplx *)P_old_in;
+    cplx *Pn = (cplx *)P_new_out;
+    size_t NN = (size_t)N * N;
+    for (int k = 0; k < K; ++k)
+        for (size_t r = 0; r < NN; ++r) {
+            real den = den_in[r];
+            Pn[k * NN + r] = (alpha + den > 0) ? (alpha * Po[k * NN + r] + num[k * NN + r]) / (alpha + den)
+                                               : Po[k * NN + r];
+        }
+}
+
+/* The frozen regularisers of oracle_set_data (A8) without a state object: the same two loops.
+ * P0 cplx [K][N][N], O0 cplx [L][H][W]; out2 = (alpha_obj, alpha_probe).                        */
+void oracle_frozen_alphas(int N, int n_views, int K, int L, int obj_h, int obj_w,
+                          const int32_t *positions, const real *P0_in, const real *O0_in,
+                          real a_obj, real a_probe, double *out2)
+{
+    const cplx *P = (const cplx *)P0_in, *O = (const cplx *)O0_in;
+    size_t NN = (size_t)N * N, HW = (size_t)obj_h * obj_w;
+    real *den = calloc(HW, sizeof(real));
+    for (int j = 0; j < n_views; ++j)
+        for (int ry = 0; ry < N; ++ry)
+            for (int rx = 0; rx < N; ++rx) {
+                real s = 0;
+                for (int k = 0; k < K; ++k) s += cabs2(P[k * NN + (size_t)ry * N + rx]);
+                den[(size_t)(positions[2 * j] + ry) * obj_w + positions[2 * j + 1] + rx] += s;
+            }
+    real mx = 0;
+    for (size_t i = 0; i < HW; ++i) if (den[i] > mx) mx = den[i];
+    out2[0] = (double)(a_obj * mx);
+    free(den);
+    mx = 0;
+    for (int ry = 0; ry < N; ++ry)
+        for (int rx = 0; rx < N; ++rx) {
+            real s = 0;
+            for (int j = 0; j < n_views; ++j)
+                for (int l = 0; l < L; ++l)
+                    s += cabs2(O[l * HW + (size_t)(positions[2 * j] + ry) * obj_w + positions[2 * j + 1] + rx]);
+            if (s > mx) mx = s;
+        }
+    out2[1] = (double)(a_probe * mx);
+}

@@ -377,3 +377,73 @@ def test_mode_power_closed_form():
     x[1] *= 3j
     assert np.allclose(oracle.mode_power(x), [0.1, 0.9])
     assert np.all(oracle.mode_power(np.zeros((3, 2, 2))) == 0.0)
+
+
+# ------------------------------------------- view-range entry points (streaming) ----
+# Justification of these oracle entry points: eqs. (5), (6) are sums over the views; carried in an
+# accumulator over consecutive view ranges they perform the additions of the monolithic functions in their order
+# (readings A3, A15).  Pin: bit-identical to oracle_object_update / oracle_probe_update / OracleDM for any split.
+@pytest.mark.parametrize("K,L", [(2, 1), (2, 2), (1, 3)])
+def test_range_accumulators_are_bit_identical_to_the_monolithic_updates(rng, K, L):
+    pos = np.array([(0, 0), (1, 5), (5, 2), (6, 8), (3, 3), (0, 7), (6, 0)], np.int32)
+    n, H, W = 8, 15, 16
+    P = rng.normal(size=(K, n, n)) + 1j * rng.normal(size=(K, n, n))
+    O = rng.normal(size=(L, H, W)) + 1j * rng.normal(size=(L, H, W))
+    psi = rng.normal(size=(len(pos), K, L, n, n)) + 1j * rng.normal(size=(len(pos), K, L, n, n))
+    for alpha in (0.0, 0.37):
+        O_ref = oracle.object_update(pos, P, psi, O, alpha)
+        P_ref = oracle.probe_update(pos, O_ref, psi, P, alpha)
+        for cuts in ([0, 7], [0, 1, 7], [0, 3, 4, 7], [0, 2, 2, 5, 7], list(range(8))):      # incl. an empty range
+            numO, denO = np.zeros((L, H, W), np.complex128), np.zeros((H, W))
+            numP, denP = np.zeros((K, n, n), np.complex128), np.zeros((n, n))
+            for j0, j1 in zip(cuts[:-1], cuts[1:]):
+                oracle.object_accumulate(pos, j0, j1, P, psi[j0:j1], numO, denO)
+            O_new = oracle.object_finish(numO, denO, O, alpha)
+            assert np.array_equal(O_new, O_ref), (alpha, cuts)
+            for j0, j1 in zip(cuts[:-1], cuts[1:]):
+                oracle.probe_accumulate(pos, j0, j1, O_new, psi[j0:j1], numP, denP)
+            assert np.array_equal(oracle.probe_finish(numP, denP, P, alpha), P_ref), (alpha, cuts)
+    # uncovered object pixels keep the old value under the literal quotient (row 14 is outside every window)
+    assert np.array_equal(oracle.object_update(pos, P, psi, O, 0.0)[:, 14], O[:, 14])
+
+
+def test_views_update_and_frozen_alphas_match_the_stateful_oracle():
+    pr = synth.make_problem(synth.CONFIGS[1].scaled(3, 4))
+    c = pr.cfg
+    o = oracle.OracleDM(c.N, c.K, c.L, c.obj_h, c.obj_w, pr.positions, beta=0.8)
+    o.set_data(pr.intensities, pr.probe0, pr.object0)
+    assert oracle.frozen_alphas(pr.positions, pr.probe0, pr.object0) == o.alphas
+    P, O, psi0 = o.probe(), o.object(), o.psi()
+    amp = np.sqrt(pr.intensities.astype(np.float64))
+    got, acc = oracle.views_update(pr.positions, 2, 9, P, O, psi0[2:9], amp[2:9], beta=0.8)
+    for j in range(2, 9):
+        y0, x0 = pr.positions[j]
+        want, a = oracle.view_update(P, O, y0, x0, psi0[j], amp[j], beta=0.8)
+        assert np.array_equal(got[j - 2], want) and np.array_equal(acc[j - 2], a)
+    o.close()
+
+
+@pytest.mark.parametrize("cfg_i,ny,nx,chunk", [(1, 3, 4, 5), (3, 2, 2, 1), (0, 4, 4, 16), (1, 3, 4, 100)])
+def test_streamed_iteration_is_bit_identical_to_oracle_iterate(cfg_i, ny, nx, chunk):
+    """tests/streamed_oracle.py (what the full-size GPU parity tests of configs 3 and 4 use) against OracleDM.iterate:
+    two iterations, the second from the state of the first, psi, P, O and the error rows bit for bit."""
+    import streamed_oracle
+    pr = synth.make_problem(synth.CONFIGS[cfg_i].scaled(ny, nx))
+    c = pr.cfg
+    o = oracle.OracleDM(c.N, c.K, c.L, c.obj_h, c.obj_w, pr.positions)
+    o.set_data(pr.intensities, pr.probe0, pr.object0)
+    a_o, a_p = oracle.frozen_alphas(pr.positions, pr.probe0, pr.object0)
+    amp = np.sqrt(pr.intensities.astype(np.float64))
+    P, O, psi = o.probe(), o.object(), o.psi()
+    for it in range(2):
+        new_psi = np.empty_like(psi)
+
+        def keep(j0, j1, chunk_psi):
+            new_psi[j0:j1] = chunk_psi
+        P, O, row = streamed_oracle.iteration(pr.positions, P, O, lambda a, b: psi[a:b], lambda a, b: amp[a:b],
+                                              a_o, a_p, chunk=chunk, on_psi=keep)
+        psi = new_psi
+        o.iterate(1)
+        assert np.array_equal(P, o.probe()) and np.array_equal(O, o.object()) and np.array_equal(psi, o.psi())
+        assert np.array_equal(row, o.errors()[it]), (row, o.errors()[it])
+    o.close()
