@@ -121,10 +121,13 @@ def test_tables_bit_exact_vs_oracle(dm, cfg_i, ny, nx):
     p.close()
 
 
-def test_tables_full_config1(dm):
-    cfg = synth.CONFIGS[1]
+@pytest.mark.parametrize("cfg_i", [1, 2, 3, 4])
+def test_tables_full_configs(dm, cfg_i):
+    """Step S0 at BASELINE.json's full sizes: window table and coverage lists bit-identical to the oracle's."""
+    cfg = synth.CONFIGS[cfg_i]
     pos = synth.make_positions(cfg, np.random.default_rng(0))
     p = dm.DMPlan(cfg.N, cfg.n_views, cfg.K, cfg.L, cfg.obj_h, cfg.obj_w, pos)
+    assert np.array_equal(p.window_table(), oracle.window_table(pos, cfg.obj_w))
     th, tw, ptr, views = p.coverage()
     optr, oviews = oracle.coverage(cfg.N, pos, cfg.obj_h, cfg.obj_w, th, tw)
     assert np.array_equal(ptr, optr) and np.array_equal(views, oviews)

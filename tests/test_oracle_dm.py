@@ -423,8 +423,20 @@ def test_views_update_and_frozen_alphas_match_the_stateful_oracle():
     o.close()
 
 
-@pytest.mark.parametrize("cfg_i,ny,nx,chunk", [(1, 3, 4, 5), (3, 2, 2, 1), (0, 4, 4, 16), (1, 3, 4, 100)])
-def test_streamed_iteration_is_bit_identical_to_oracle_iterate(cfg_i, ny, nx, chunk):
+class _DictStash:
+    def __init__(self):
+        self.d = {}
+
+    def put(self, j0, j1, x):
+        self.d[(j0, j1)] = x.copy()
+
+    def get(self, j0, j1):
+        return self.d[(j0, j1)]
+
+
+@pytest.mark.parametrize("cfg_i,ny,nx,chunk,use_stash", [(1, 3, 4, 5, False), (3, 2, 2, 1, True), (0, 4, 4, 16, False),
+                                                         (1, 3, 4, 100, True), (1, 3, 4, 5, True)])
+def test_streamed_iteration_is_bit_identical_to_oracle_iterate(cfg_i, ny, nx, chunk, use_stash):
     """tests/streamed_oracle.py (what the full-size GPU parity tests of configs 3 and 4 use) against OracleDM.iterate:
     two iterations, the second from the state of the first, psi, P, O and the error rows bit for bit."""
     import streamed_oracle
@@ -441,7 +453,8 @@ def test_streamed_iteration_is_bit_identical_to_oracle_iterate(cfg_i, ny, nx, ch
         def keep(j0, j1, chunk_psi):
             new_psi[j0:j1] = chunk_psi
         P, O, row = streamed_oracle.iteration(pr.positions, P, O, lambda a, b: psi[a:b], lambda a, b: amp[a:b],
-                                              a_o, a_p, chunk=chunk, on_psi=keep)
+                                              a_o, a_p, chunk=chunk, on_psi=keep,
+                                              stash=_DictStash() if use_stash else None)
         psi = new_psi
         o.iterate(1)
         assert np.array_equal(P, o.probe()) and np.array_equal(O, o.object()) and np.array_equal(psi, o.psi())
